@@ -1,0 +1,179 @@
+/* dgrtm.h - C ABI of libdgrtm: nodal discontinuous Galerkin time-domain (DGTD) acoustic solver and
+ * reverse-time migration (RTM) on unstructured tetrahedra, hand-written CUDA for sm_100a (B200).
+ *
+ * Method: Modave, St-Cyr, Mulder, Warburton, arXiv 1506.00907 ("the paper"; PAPER.md = its text).
+ * Every entry point cites the passage that defines the operation.  Readings of silent / garbled
+ * passages are numbered Q1..Q16 in DESIGN.md.
+ *
+ * Conventions
+ *  - plain C, opaque handle dg_ctx*.  Every call returns int: 0 = OK, negative = error code below;
+ *    dg_last_error(ctx) returns a message owned by the ctx.  No exception or abort crosses the ABI.
+ *  - HOST pointers everywhere except dg_bind_workspace / rtm_bind_history, which take DEVICE pointers
+ *    (the caller owns device memory, e.g. a torch uint8 tensor) and a cudaStream_t passed as void*.
+ *  - input arrays are borrowed for the duration of the call and copied; outputs go to caller-allocated
+ *    buffers.  Indices are 0-based int32.  Coordinates, material and field values cross the ABI as
+ *    double regardless of the compute precision (rounded once inside).
+ *  - element order and node order of every array crossing the ABI is the USER's (the order of EToV
+ *    and of dg_get_nodes); the internal level-sorted, 32-element-blocked layout never shows.
+ *  - field layout q[k][field][n], field 0 = p, 1..3 = v_x, v_y, v_z (eqs (1)-(2)).
+ *  - levels: 0 = coarsest (the paper's l = 1) .. L-1 = finest.
+ *  - all kernels are enqueued on the bound stream; calls that return data synchronise that stream.
+ *  - a ctx is not thread-safe; distinct ctxs are independent.
+ */
+#ifndef DGRTM_H
+#define DGRTM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dg_ctx dg_ctx;
+
+enum {
+  DG_OK = 0,
+  DG_ERR_ARG = -1,         /* NULL / out-of-range argument or size */
+  DG_ERR_MESH = -2,        /* degenerate, negatively oriented or non-conforming mesh */
+  DG_ERR_STATE = -3,       /* call out of order (e.g. dg_step before dg_set_model / bind) */
+  DG_ERR_CUDA = -4,        /* CUDA runtime error (message in dg_last_error) */
+  DG_ERR_NOMEM = -5,       /* bound workspace / history too small */
+  DG_ERR_UNSUPPORTED = -6  /* N outside 1..6, precision not 32/64, ... */
+};
+
+/* boundary-condition types of a boundary face (eq (3); exterior states: reading Q6) */
+enum { DG_BC_FREE = 1, DG_BC_ABSORBING = 2, DG_BC_RIGID = 3, DG_BC_PRESCRIBED = 4 };
+enum { DG_INTEGRATOR_AB3 = 0, DG_INTEGRATOR_LSERK4 = 1 };
+enum { DG_WAVELET_RICKER = 0 };
+enum { DG_IMAGING_CLASSICAL = 0, DG_IMAGING_CHARACTERISTIC = 1 };
+enum { DG_RHS_VOLUME = 0, DG_RHS_SURFACE = 1, DG_RHS_TOTAL = 2 };
+
+const char* dg_version(void);
+/* Message of the last failed call on this ctx (or of the last failed dg_mesh_create if ctx==NULL). */
+const char* dg_last_error(const dg_ctx* ctx);
+
+/* ---- setup -------------------------------------------------------------------------------------
+ * dg_mesh_create: nodal DG space of order N (N_p=(N+1)(N+2)(N+3)/6 warp-and-blend nodes, eqs (9)-(10)
+ * PAPER.md:84-96) on the K tetrahedra EToV[K][4] with vertices VX[Nv][3]; builds D_r,D_s,D_t, L_f
+ * (App. A 593-612), geometric factors (App. A 606-624, reading Q3), face connectivity
+ * and the boundary-face list (host, fp64).  precision = 32 or 64 selects the device arithmetic.
+ * face_bc[K][4] (may be NULL) gives the type of each BOUNDARY face (0 -> default_bc); entries of
+ * interior faces are ignored.  Tets with non-positive volume -> DG_ERR_MESH (never re-ordered). */
+int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, const int32_t* EToV,
+                   const double* VX, const int8_t* face_bc, int default_bc);
+void dg_destroy(dg_ctx* ctx);
+
+/* dg_set_model: piecewise-constant rho[K], c[K] (replaces phyDB/phyMap PAPER.md:258).
+ * dt_k = cfl*l_k/((N+1)^2 c_k), dt_local = min_k dt_k, multi-rate levels with at most
+ * one level between face neighbours (reading Q9), level-sorted device layout.
+ * nlevels = 1 -> single rate.  Must precede dg_workspace_bytes. */
+int dg_set_model(dg_ctx* ctx, const double* rho, const double* c, int nlevels, double cfl);
+/* AB3 / multi-rate AB3 (eqs (18)-(19) PAPER.md:156-166, Alg. 1; default) or the
+ * five-stage LSERK4 (not in the paper; BASELINE.json config 1, reading Q8; single rate only). */
+int dg_set_integrator(dg_ctx* ctx, int integrator);
+/* Overrides dt_local (default: the CFL value of dg_set_model).  Testing aid (convergence in dt). */
+int dg_set_dt(dg_ctx* ctx, double dt_local);
+
+/* Point source f(t) delta(x-x0) L2-projected on the element containing x0 (eq (15) PAPER.md:122-128,
+ * scaling of eq (1): reading Q5; owner element: reading Q11).  Ricker f(t) = amp (1-2a) exp(-a),
+ * a = (pi f0 (t-tp))^2. */
+int dg_set_source(dg_ctx* ctx, const double x0[3], int wavelet, double f0, double tp, double amp);
+/* nr receivers xr[nr][3]: sampling rows l_n(x_r) and injection weights M_k^-1 l(x_r) (eq (15)). */
+int dg_set_receivers(dg_ctx* ctx, int64_t nr, const double* xr);
+
+/* Device memory.  The library allocates none: query, allocate (e.g. a torch tensor), bind.
+ * dptr must be 256-byte aligned device memory of at least n bytes that stays valid until dg_destroy
+ * or the next bind; stream is a cudaStream_t (NULL = legacy default stream).  Binding uploads all
+ * tables and zeroes the fields (state = rest at t = 0). */
+int dg_workspace_bytes(dg_ctx* ctx, size_t* n);
+int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream);
+
+/* ---- time stepping ------------------------------------------------------------------------------
+ * dg_set_state: nodal fields q[K][4][Np] at time t0; right-hand-side history cleared (AB start-up by
+ * AB1, AB2: reading Q7); exposed traces (p, n.v) refreshed. */
+int dg_set_state(dg_ctx* ctx, const double* q, double t0);
+/* Advance nsteps GLOBAL steps (= 2^(L-1) fine steps of dt_local each) forward in time with the point
+ * source on (if set): per fine step the volume + surface right-hand side (eqs (13)-(14) PAPER.md:
+ * 113-118, penalties (11)-(12) PAPER.md:100-111, Algs 2-3) of the levels that sit at the step start,
+ * the update (18) of the levels that land on the step end and the half-step traces (19) of their
+ * not-updated coarse neighbours (Alg. 1, Alg. 4).  Asynchronous on the stream. */
+int dg_step(dg_ctx* ctx, int nsteps);
+/* Prescribed-exterior faces (DG_BC_PRESCRIBED; plane-wave tests): exterior traces (p+, n.v+ with the
+ * owner's outward normal) ext[nbnd][Nfp][2] in boundary-face-list order, used by every following
+ * right-hand side until replaced.  Entries of faces of another type are ignored. */
+int dg_set_exterior(dg_ctx* ctx, const double* ext);
+
+/* ---- RTM (Fig. 1) ---------------------------------------------------
+ * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side
+ * evaluation time of its owner plus the final time (layout reading Q12) - it stays in
+ * HBM.  rtm_history_bytes: size for shots of nsteps global steps. */
+int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n);
+int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n);
+/* Forward phase: from rest at t = 0, source on, nsteps global steps; captures the boundary traces,
+ * keeps q(t_f) on the device, records p(x_r, j dt_local), j = 0..nfine, into data_out[nr][nfine+1]
+ * (host; may be NULL).  Synchronises. */
+int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out);
+/* Backward phase: source field reconstructed from q(t_f) with the stored traces as exterior states,
+ * receiver field from rest with data[nr][nfine+1] injected (eq (15) weights), both stepped backward
+ * in time with negative penalty parameters; before every update the step's
+ * contribution to the image is accumulated with the AB-consistent integral (eqs (20)-(24) PAPER.md:
+ * 174-204, corrected coefficients: reading Q1, sign: Q1b) of the classical (eq (4)) or
+ * the characteristic pressure+velocity condition q_S^- q_R^+, q^+- = p +- c rho e.v (eqs (5)-(8)
+ * PAPER.md:55-68), e = updir.  Only steps whose start index (forward numbering of global steps) is
+ * > first_image_step contribute... i.e. imaging over t in [first_image_step*dt_global, t_f]
+ * (PAPER.md:460).  Images of successive shots add up.  Synchronises. */
+int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double updir[3],
+                      int imaging, int64_t first_image_step);
+int rtm_image_read(dg_ctx* ctx, double* I_out /* [K][Np] */);
+int rtm_image_zero(dg_ctx* ctx);
+
+/* ---- getters (parity checks; all synchronise) ----------------------------------------------------*/
+int dg_get_sizes(const dg_ctx* ctx, int64_t* K, int* Np, int* Nfp, int64_t* nbnd, int64_t* nr);
+int dg_get_nodes(const dg_ctx* ctx, double* r, double* s, double* t /* [Np] each */);
+/* Dr,Ds,Dt [Np][Np]; LIFT [Np][4*Nfp] (column block f = L_f); Fmask [4][Nfp].  NULL = skip. */
+int dg_get_operators(const dg_ctx* ctx, double* Dr, double* Ds, double* Dt, double* LIFT,
+                     int32_t* Fmask);
+/* EToE, EToF [K][4] (-1 on boundary faces); mapP [K][4][Nfp]: face-node index on the neighbour face
+ * that coincides with face node i (identity on boundary faces).  NULL = skip. */
+int dg_get_connectivity(const dg_ctx* ctx, int32_t* EToE, int32_t* EToF, int32_t* mapP);
+/* Boundary-face list (ascending (k,f)): element, local face, type.  [nbnd] each, NULL = skip. */
+int dg_get_boundary_faces(const dg_ctx* ctx, int32_t* bk, int32_t* bf, int32_t* bc);
+/* J [K], ginv [K][3][3] (= d r_j / d x_i), normals [K][4][3], gsur [K][4], ell [K].  NULL = skip. */
+int dg_get_geometry(const dg_ctx* ctx, double* J, double* ginv, double* normals, double* gsur,
+                    double* ell);
+int dg_get_levels(const dg_ctx* ctx, int32_t* level /* [K] */);
+int dg_get_dt(const dg_ctx* ctx, double* dt_local, int* nlocal /* fine steps per global step */);
+int dg_get_time(const dg_ctx* ctx, double* t);
+int dg_get_source(const dg_ctx* ctx, int32_t* k, double* w /* [Np] */);
+int dg_get_receivers(const dg_ctx* ctx, int32_t* k /* [nr] */, double* rows /* [nr][Np] */,
+                     double* w /* [nr][Np] */);
+int dg_get_fields(dg_ctx* ctx, double* q /* [K][4][Np] */);
+/* Exposed traces qf[K][4][Nfp][2] = (p, n.v) in the OWNER's face-node order. */
+int dg_get_traces(dg_ctx* ctx, double* qf);
+/* Right-hand side of the current state at the current time, evaluated now by the volume kernel, the
+ * surface kernel or both (no source term); r[K][4][Np].  Does not advance or disturb the state.
+ * direction = +1 / -1 (sign of the penalty parameters). */
+int dg_get_rhs(dg_ctx* ctx, int which, int direction, double* r);
+/* RTM bookkeeping: per level, the boundary-face-list indices of the stored faces (ascending) and the
+ * number of records.  faces may be NULL to query nfaces / nrecords only. */
+int rtm_get_trace_index(const dg_ctx* ctx, int level, int64_t* nfaces, int64_t* nrecords,
+                        int32_t* faces);
+/* Record j of a level: buf[nfaces][Nfp][2] = (p, n.v). */
+int rtm_get_traces(dg_ctx* ctx, int level, int64_t record, double* buf);
+/* Wavefields kept by the RTM phases: which = 0 final forward state q(t_f), 1 = reconstructed source
+ * field, 2 = receiver field (the latter two after rtm_backward_shot). */
+int rtm_get_fields(dg_ctx* ctx, int which, double* q /* [K][4][Np] */);
+
+/* ---- measurement ------------------------------------------------------------------------------
+ * Counts of kernels launched by this ctx since creation (bench.py's gpu_launches). */
+int dg_get_launch_count(const dg_ctx* ctx, int64_t* n);
+/* Enqueue `reps` launches of one kernel over the whole mesh on the bound stream (state is disturbed:
+ * for kernel timing only).  which: 0 volume, 1 surface, 2 fused volume+surface, 3 update (18),
+ * 4 backward update with fused imaging (two wavefields). */
+int dg_bench_kernel(dg_ctx* ctx, int which, int reps);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DGRTM_H */

@@ -1,0 +1,332 @@
+"""Thin ctypes binding of libdgrtm.so (include/dgrtm.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch supplies device memory
+(uint8 tensors) and the stream, nothing else.  There is no CPU fallback: if the library is missing
+the import of this module fails.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdgrtm.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        "libdgrtm.so is not built: run `python -m paper_1506_00907_b200.build` "
+        "(there is no CPU fallback for the DGTD hot path)")
+_lib = C.CDLL(LIB_PATH)
+
+DG_OK = 0
+DG_ERR_ARG, DG_ERR_MESH, DG_ERR_STATE, DG_ERR_CUDA, DG_ERR_NOMEM, DG_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
+DG_BC_FREE, DG_BC_ABSORBING, DG_BC_RIGID, DG_BC_PRESCRIBED = 1, 2, 3, 4
+DG_INTEGRATOR_AB3, DG_INTEGRATOR_LSERK4 = 0, 1
+DG_WAVELET_RICKER = 0
+DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
+DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
+
+_vp, _i, _i64, _d, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_size_t
+_pd = C.POINTER(C.c_double)
+_pi32 = C.POINTER(C.c_int32)
+_pi8 = C.POINTER(C.c_int8)
+_pi64 = C.POINTER(C.c_int64)
+_pint = C.POINTER(C.c_int)
+_psz = C.POINTER(C.c_size_t)
+
+# name -> (restype, argtypes): the complete export list of include/dgrtm.h
+SIGNATURES = {
+    "dg_version": (C.c_char_p, []),
+    "dg_last_error": (C.c_char_p, [_vp]),
+    "dg_mesh_create": (_i, [C.POINTER(_vp), _i, _i, _i64, _i64, _pi32, _pd, _pi8, _i]),
+    "dg_destroy": (None, [_vp]),
+    "dg_set_model": (_i, [_vp, _pd, _pd, _i, _d]),
+    "dg_set_integrator": (_i, [_vp, _i]),
+    "dg_set_dt": (_i, [_vp, _d]),
+    "dg_set_source": (_i, [_vp, _pd, _i, _d, _d, _d]),
+    "dg_set_receivers": (_i, [_vp, _i64, _pd]),
+    "dg_workspace_bytes": (_i, [_vp, _psz]),
+    "dg_bind_workspace": (_i, [_vp, _vp, _sz, _vp]),
+    "dg_set_state": (_i, [_vp, _pd, _d]),
+    "dg_step": (_i, [_vp, _i]),
+    "dg_set_exterior": (_i, [_vp, _pd]),
+    "rtm_history_bytes": (_i, [_vp, _i, _psz]),
+    "rtm_bind_history": (_i, [_vp, _vp, _sz]),
+    "rtm_forward_shot": (_i, [_vp, _i, _pd]),
+    "rtm_backward_shot": (_i, [_vp, _i, _pd, _pd, _i, _i64]),
+    "rtm_image_read": (_i, [_vp, _pd]),
+    "rtm_image_zero": (_i, [_vp]),
+    "dg_get_sizes": (_i, [_vp, _pi64, _pint, _pint, _pi64, _pi64]),
+    "dg_get_nodes": (_i, [_vp, _pd, _pd, _pd]),
+    "dg_get_operators": (_i, [_vp, _pd, _pd, _pd, _pd, _pi32]),
+    "dg_get_connectivity": (_i, [_vp, _pi32, _pi32, _pi32]),
+    "dg_get_boundary_faces": (_i, [_vp, _pi32, _pi32, _pi32]),
+    "dg_get_geometry": (_i, [_vp, _pd, _pd, _pd, _pd, _pd]),
+    "dg_get_levels": (_i, [_vp, _pi32]),
+    "dg_get_dt": (_i, [_vp, _pd, _pint]),
+    "dg_get_time": (_i, [_vp, _pd]),
+    "dg_get_source": (_i, [_vp, _pi32, _pd]),
+    "dg_get_receivers": (_i, [_vp, _pi32, _pd, _pd]),
+    "dg_get_fields": (_i, [_vp, _pd]),
+    "dg_get_traces": (_i, [_vp, _pd]),
+    "dg_get_rhs": (_i, [_vp, _i, _i, _pd]),
+    "rtm_get_trace_index": (_i, [_vp, _i, _pi64, _pi64, _pi32]),
+    "rtm_get_traces": (_i, [_vp, _i, _i64, _pd]),
+    "rtm_get_fields": (_i, [_vp, _i, _pd]),
+    "dg_get_launch_count": (_i, [_vp, _pi64]),
+    "dg_bench_kernel": (_i, [_vp, _i, _i]),
+}
+for _name, (_res, _args) in SIGNATURES.items():
+    _fn = getattr(_lib, _name)
+    _fn.restype = _res
+    _fn.argtypes = _args
+
+
+class DGError(RuntimeError):
+    def __init__(self, code, message):
+        super().__init__("libdgrtm error %d: %s" % (code, message))
+        self.code = code
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr(a, typ):
+    return None if a is None else a.ctypes.data_as(typ)
+
+
+class DG:
+    """One dg_ctx.  Method names are the C entry points without the dg_/rtm_ split removed:
+    dg_mesh_create is the constructor; every other call is a method of the same name."""
+
+    def __init__(self, N, precision, EToV, VX, face_bc=None, default_bc=DG_BC_ABSORBING):
+        etov = np.ascontiguousarray(EToV, dtype=np.int32)
+        vx = _f64(VX)
+        fb = None if face_bc is None else np.ascontiguousarray(face_bc, dtype=np.int8)
+        self._h = _vp()
+        rc = _lib.dg_mesh_create(C.byref(self._h), int(N), int(precision), etov.shape[0], vx.shape[0],
+                                 _ptr(etov, _pi32), _ptr(vx, _pd), _ptr(fb, _pi8), int(default_bc))
+        if rc != DG_OK:
+            raise DGError(rc, (_lib.dg_last_error(None) or b"").decode())
+        self.N, self.precision = int(N), int(precision)
+        K, Np, Nfp, nbnd, nr = _i64(), _i(), _i(), _i64(), _i64()
+        _lib.dg_get_sizes(self._h, C.byref(K), C.byref(Np), C.byref(Nfp), C.byref(nbnd), C.byref(nr))
+        self.K, self.Np, self.Nfp, self.nbnd = K.value, Np.value, Nfp.value, nbnd.value
+        self.nr = 0
+        self._ws = None
+        self._hist = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.dg_destroy(self._h)
+            self._h = None
+        self._ws = None
+        self._hist = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != DG_OK:
+            raise DGError(rc, (_lib.dg_last_error(self._h) or b"").decode())
+
+    # ---- setup
+    def dg_set_model(self, rho, c, nlevels=1, cfl=0.15):
+        rho, c = _f64(rho), _f64(c)
+        assert rho.shape == (self.K,) and c.shape == (self.K,)
+        self._ck(_lib.dg_set_model(self._h, _ptr(rho, _pd), _ptr(c, _pd), int(nlevels), float(cfl)))
+
+    def dg_set_integrator(self, integrator):
+        self._ck(_lib.dg_set_integrator(self._h, int(integrator)))
+
+    def dg_set_dt(self, dt_local):
+        self._ck(_lib.dg_set_dt(self._h, float(dt_local)))
+
+    def dg_set_source(self, x0, f0, tp, amp=1.0, wavelet=DG_WAVELET_RICKER):
+        x0 = _f64(x0)
+        self._ck(_lib.dg_set_source(self._h, _ptr(x0, _pd), int(wavelet), float(f0), float(tp), float(amp)))
+
+    def dg_set_receivers(self, xr):
+        xr = _f64(xr).reshape(-1, 3)
+        self._ck(_lib.dg_set_receivers(self._h, xr.shape[0], _ptr(xr, _pd)))
+        self.nr = xr.shape[0]
+
+    def dg_workspace_bytes(self):
+        n = _sz()
+        self._ck(_lib.dg_workspace_bytes(self._h, C.byref(n)))
+        return n.value
+
+    def dg_bind_workspace(self, dptr, nbytes, stream=0):
+        self._ck(_lib.dg_bind_workspace(self._h, _vp(dptr), nbytes, _vp(stream)))
+
+    def bind_torch(self, device="cuda:0", stream=None):
+        """Allocates the workspace as a torch uint8 tensor and binds it with torch's current stream."""
+        import torch
+        n = self.dg_workspace_bytes()
+        self._ws = torch.empty(n + 256, dtype=torch.uint8, device=device)
+        base = (self._ws.data_ptr() + 255) & ~255
+        s = stream if stream is not None else torch.cuda.current_stream(device).cuda_stream
+        self.dg_bind_workspace(base, n, s)
+        return n
+
+    # ---- stepping
+    def dg_set_state(self, q, t0=0.0):
+        q = _f64(q)
+        assert q.shape == (self.K, 4, self.Np)
+        self._ck(_lib.dg_set_state(self._h, _ptr(q, _pd), float(t0)))
+
+    def dg_step(self, nsteps):
+        self._ck(_lib.dg_step(self._h, int(nsteps)))
+
+    def dg_set_exterior(self, ext):
+        ext = _f64(ext)
+        assert ext.shape == (self.nbnd, self.Nfp, 2)
+        self._ck(_lib.dg_set_exterior(self._h, _ptr(ext, _pd)))
+
+    # ---- RTM
+    def rtm_history_bytes(self, nsteps):
+        n = _sz()
+        self._ck(_lib.rtm_history_bytes(self._h, int(nsteps), C.byref(n)))
+        return n.value
+
+    def rtm_bind_history(self, dptr, nbytes):
+        self._ck(_lib.rtm_bind_history(self._h, _vp(dptr), nbytes))
+
+    def bind_history_torch(self, nsteps, device="cuda:0"):
+        import torch
+        n = self.rtm_history_bytes(nsteps)
+        self._hist = torch.empty(n + 256, dtype=torch.uint8, device=device)
+        base = (self._hist.data_ptr() + 255) & ~255
+        self.rtm_bind_history(base, n)
+        return n
+
+    def rtm_forward_shot(self, nsteps, want_data=True):
+        nloc = self.dg_get_dt()[1]
+        data = np.empty((self.nr, nsteps * nloc + 1)) if (want_data and self.nr) else None
+        self._ck(_lib.rtm_forward_shot(self._h, int(nsteps), _ptr(data, _pd)))
+        return data
+
+    def rtm_backward_shot(self, nsteps, data, updir=(0.0, 0.0, -1.0), imaging=DG_IMAGING_CHARACTERISTIC,
+                          first_image_step=0):
+        d = None if data is None else _f64(data)
+        u = _f64(updir)
+        self._ck(_lib.rtm_backward_shot(self._h, int(nsteps), _ptr(d, _pd), _ptr(u, _pd), int(imaging),
+                                        int(first_image_step)))
+
+    def rtm_image_read(self):
+        out = np.empty((self.K, self.Np))
+        self._ck(_lib.rtm_image_read(self._h, _ptr(out, _pd)))
+        return out
+
+    def rtm_image_zero(self):
+        self._ck(_lib.rtm_image_zero(self._h))
+
+    # ---- getters
+    def dg_get_nodes(self):
+        r, s, t = (np.empty(self.Np) for _ in range(3))
+        self._ck(_lib.dg_get_nodes(self._h, _ptr(r, _pd), _ptr(s, _pd), _ptr(t, _pd)))
+        return r, s, t
+
+    def dg_get_operators(self):
+        Np, Nfp = self.Np, self.Nfp
+        Dr, Ds, Dt = (np.empty((Np, Np)) for _ in range(3))
+        LIFT = np.empty((Np, 4 * Nfp))
+        Fmask = np.empty((4, Nfp), dtype=np.int32)
+        self._ck(_lib.dg_get_operators(self._h, _ptr(Dr, _pd), _ptr(Ds, _pd), _ptr(Dt, _pd), _ptr(LIFT, _pd),
+                                       _ptr(Fmask, _pi32)))
+        return Dr, Ds, Dt, LIFT, Fmask
+
+    def dg_get_connectivity(self):
+        EToE = np.empty((self.K, 4), dtype=np.int32)
+        EToF = np.empty((self.K, 4), dtype=np.int32)
+        mapP = np.empty((self.K, 4, self.Nfp), dtype=np.int32)
+        self._ck(_lib.dg_get_connectivity(self._h, _ptr(EToE, _pi32), _ptr(EToF, _pi32), _ptr(mapP, _pi32)))
+        return EToE, EToF, mapP
+
+    def dg_get_boundary_faces(self):
+        bk, bf, bc = (np.empty(self.nbnd, dtype=np.int32) for _ in range(3))
+        self._ck(_lib.dg_get_boundary_faces(self._h, _ptr(bk, _pi32), _ptr(bf, _pi32), _ptr(bc, _pi32)))
+        return bk, bf, bc
+
+    def dg_get_geometry(self):
+        K = self.K
+        J, ginv, nrm, gsur, ell = np.empty(K), np.empty((K, 3, 3)), np.empty((K, 4, 3)), np.empty((K, 4)), np.empty(K)
+        self._ck(_lib.dg_get_geometry(self._h, _ptr(J, _pd), _ptr(ginv, _pd), _ptr(nrm, _pd), _ptr(gsur, _pd),
+                                      _ptr(ell, _pd)))
+        return dict(J=J, ginv=ginv, normals=nrm, gsur=gsur, ell=ell)
+
+    def dg_get_levels(self):
+        lv = np.empty(self.K, dtype=np.int32)
+        self._ck(_lib.dg_get_levels(self._h, _ptr(lv, _pi32)))
+        return lv
+
+    def dg_get_dt(self):
+        dt, nl = _d(), _i()
+        self._ck(_lib.dg_get_dt(self._h, C.byref(dt), C.byref(nl)))
+        return dt.value, nl.value
+
+    def dg_get_time(self):
+        t = _d()
+        self._ck(_lib.dg_get_time(self._h, C.byref(t)))
+        return t.value
+
+    def dg_get_source(self):
+        k = C.c_int32()
+        w = np.empty(self.Np)
+        self._ck(_lib.dg_get_source(self._h, C.byref(k), _ptr(w, _pd)))
+        return k.value, w
+
+    def dg_get_receivers(self):
+        k = np.empty(self.nr, dtype=np.int32)
+        rows, w = np.empty((self.nr, self.Np)), np.empty((self.nr, self.Np))
+        self._ck(_lib.dg_get_receivers(self._h, _ptr(k, _pi32), _ptr(rows, _pd), _ptr(w, _pd)))
+        return k, rows, w
+
+    def dg_get_fields(self):
+        q = np.empty((self.K, 4, self.Np))
+        self._ck(_lib.dg_get_fields(self._h, _ptr(q, _pd)))
+        return q
+
+    def dg_get_traces(self):
+        qf = np.empty((self.K, 4, self.Nfp, 2))
+        self._ck(_lib.dg_get_traces(self._h, _ptr(qf, _pd)))
+        return qf
+
+    def dg_get_rhs(self, which=DG_RHS_TOTAL, direction=1):
+        r = np.empty((self.K, 4, self.Np))
+        self._ck(_lib.dg_get_rhs(self._h, int(which), int(direction), _ptr(r, _pd)))
+        return r
+
+    def rtm_get_trace_index(self, level):
+        nf, nrec = _i64(), _i64()
+        self._ck(_lib.rtm_get_trace_index(self._h, int(level), C.byref(nf), C.byref(nrec), None))
+        faces = np.empty(nf.value, dtype=np.int32)
+        self._ck(_lib.rtm_get_trace_index(self._h, int(level), C.byref(nf), C.byref(nrec), _ptr(faces, _pi32)))
+        return faces, nrec.value
+
+    def rtm_get_traces(self, level, record):
+        nf = self.rtm_get_trace_index(level)[0].size
+        buf = np.empty((nf, self.Nfp, 2))
+        self._ck(_lib.rtm_get_traces(self._h, int(level), int(record), _ptr(buf, _pd)))
+        return buf
+
+    def rtm_get_fields(self, which):
+        q = np.empty((self.K, 4, self.Np))
+        self._ck(_lib.rtm_get_fields(self._h, int(which), _ptr(q, _pd)))
+        return q
+
+    def dg_get_launch_count(self):
+        n = _i64()
+        self._ck(_lib.dg_get_launch_count(self._h, C.byref(n)))
+        return n.value
+
+    def dg_bench_kernel(self, which, reps):
+        self._ck(_lib.dg_bench_kernel(self._h, int(which), int(reps)))
+
+
+def dg_version():
+    return _lib.dg_version().decode()

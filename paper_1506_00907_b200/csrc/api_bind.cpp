@@ -1,0 +1,141 @@
+// C ABI of libdgrtm, part 2: binding caller-owned device memory, uploading the tables of the
+// level-sorted, 32-element-blocked layout (kernels.h), initial state.
+#include <algorithm>
+
+#include "ctx.h"
+
+using namespace dgrtm;
+
+namespace {
+
+void upload_tables(dg_ctx* c) {
+  const int Np = c->Np, Nfp = c->Nfp, NF = c->NF;
+  const RefElem& re = c->re;
+  const Mesh& m = c->mesh;
+  const Model& md = c->model;
+  // operators, transposed for the kernels: D3T[m][n][3] = D_{r,s,t}[n][m]; LIFTT[j][n] = LIFT[n][j]
+  std::vector<double> D3T((size_t)3 * Np * Np), LT((size_t)NF * Np);
+  for (int mm = 0; mm < Np; ++mm)
+    for (int n = 0; n < Np; ++n) {
+      D3T[((size_t)mm * Np + n) * 3 + 0] = re.Dr[(size_t)n * Np + mm];
+      D3T[((size_t)mm * Np + n) * 3 + 1] = re.Ds[(size_t)n * Np + mm];
+      D3T[((size_t)mm * Np + n) * 3 + 2] = re.Dt[(size_t)n * Np + mm];
+    }
+  for (int j = 0; j < NF; ++j)
+    for (int n = 0; n < Np; ++n) LT[(size_t)j * Np + n] = re.LIFT[(size_t)n * NF + j];
+  upload_real(c, const_cast<void*>(c->ops.D3T), D3T.data(), D3T.size());
+  upload_real(c, const_cast<void*>(c->ops.LIFTT), LT.data(), LT.size());
+  upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);
+  upload_raw(c, const_cast<int*>(c->ops.ptab), m.ptab.data(), m.ptab.size() * 4);
+
+  // position of every stored (absorbing) boundary face inside its level's record
+  std::vector<int32_t> stored_pos(m.bnd_k.size(), 0);
+  for (int l = 0; l < md.nlevels; ++l)
+    for (size_t x = 0; x < md.stored[l].size(); ++x) stored_pos[md.stored[l][x]] = (int32_t)x;
+
+  const int64_t nb = md.nblocks;
+  std::vector<double> geo((size_t)nb * DG_NGEO * 32, 0.0);
+  std::vector<int32_t> nbr((size_t)nb * 4 * 32, -1), wperm((size_t)nb * 32, 0);
+  for (int64_t s = 0; s < md.nslots; ++s) {
+    const int64_t k = md.elem_of[s], b = s >> 5, lane = s & 31;
+    double* g = &geo[(size_t)b * DG_NGEO * 32 + lane];
+    if (k < 0) {                                   // padding slot: inert
+      for (int f = 0; f < 4; ++f) g[(GEO_FACE + 5 * f + 4) * 32] = 1.0;
+      g[GEO_IRHO * 32] = 1.0;
+      continue;
+    }
+    const double rho = md.rho[k], cc = md.c[k], Z = rho * cc;
+    for (int x = 0; x < 9; ++x) g[(GEO_G + x) * 32] = m.ginv[9 * k + x];
+    g[GEO_RC2 * 32] = rho * cc * cc;
+    g[GEO_IRHO * 32] = 1.0 / rho;
+    g[GEO_Z * 32] = Z;
+    int wp = 0;
+    for (int f = 0; f < 4; ++f) {
+      const int64_t k2 = m.EToE[4 * k + f];
+      for (int d = 0; d < 3; ++d) g[(GEO_FACE + 5 * f + d) * 32] = m.normals[12 * k + 3 * f + d];
+      g[(GEO_FACE + 5 * f + 3) * 32] = m.gsur[4 * k + f];
+      // single-valued face impedance (reading Q4)
+      g[(GEO_FACE + 5 * f + 4) * 32] = k2 >= 0 ? 0.5 * (Z + md.rho[k2] * md.c[k2]) : Z;
+      int32_t code;
+      if (k2 >= 0) {
+        code = (int32_t)(md.slot_of[k2] * 4 + m.EToF[4 * k + f]);
+      } else {
+        const int bc = m.bc[4 * k + f];
+        const int32_t bi = m.bnd_index[4 * k + f];
+        const int64_t bpos = bc == DG_BC_ABSORBING ? stored_pos[bi] : (bc == DG_BC_PRESCRIBED ? bi : 0);
+        code = (int32_t)(-1 - (bpos * 8 + bc));
+      }
+      nbr[((size_t)b * 4 + f) * 32 + lane] = code;
+      wp |= (int)m.perm_id[4 * k + f] << (8 * f);
+    }
+    wperm[s] = wp;
+  }
+  upload_real(c, c->geo, geo.data(), geo.size());
+  upload_raw(c, c->nbr, nbr.data(), nbr.size() * 4);
+  upload_raw(c, c->wperm, wperm.data(), wperm.size() * 4);
+
+  for (int l = 0; l < md.nlevels; ++l) {
+    upload_raw(c, c->d_coarse[l], md.coarse_nb[l].data(), md.coarse_nb[l].size() * 4);
+    std::vector<int32_t> sf(md.stored[l].size());
+    for (size_t x = 0; x < sf.size(); ++x) {
+      const int32_t bi = md.stored[l][x];
+      sf[x] = (int32_t)(md.slot_of[m.bnd_k[bi]] * 4 + m.bnd_f[bi]);
+    }
+    upload_raw(c, c->d_stored[l], sf.data(), sf.size() * 4);
+  }
+  if (c->has_src) upload_real(c, c->d_src_w, c->src_w.data(), Np);
+}
+
+}  // namespace
+
+extern "C" {
+
+int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream) {
+  DG_TRY(ctx)
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  if (!dptr) throw ApiError(DG_ERR_ARG, "device pointer is NULL");
+  if (((uintptr_t)dptr & 255) != 0) throw ApiError(DG_ERR_ARG, "device pointer must be 256-byte aligned");
+  size_t need = 0;
+  int rc = dg_workspace_bytes(ctx, &need);
+  if (rc != DG_OK) return rc;
+  if (n < need) throw ApiError(DG_ERR_NOMEM, "workspace too small: need " + std::to_string(need) + " bytes");
+  if (!ctx->kt) throw ApiError(DG_ERR_UNSUPPORTED, "no kernels for this order / precision");
+  const int e = ctx->kt->init();
+  if (e != 0) throw ApiError(DG_ERR_CUDA, std::string("kernel attribute setup: ") + cudaGetErrorString((cudaError_t)e));
+  ctx->ws = (char*)dptr; ctx->ws_bytes = n; ctx->stream = (cudaStream_t)cuda_stream;
+  Carver cv;
+  cv.base = ctx->ws;
+  carve_workspace(ctx, cv);
+  ctx->bound = true; ctx->hist_bound = false;
+  cuda_check(cudaMemsetAsync(ctx->ws, 0, need, ctx->stream), "cudaMemsetAsync workspace");
+  upload_tables(ctx);
+  ctx->F.reset_history();
+  ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false;
+  ctx->have_final = false; ctx->have_backward = false;
+  sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+int dg_set_state(dg_ctx* ctx, const double* q, double t0) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!q) throw ApiError(DG_ERR_ARG, "q is NULL");
+  clear_field(ctx, ctx->F);
+  cuda_check(cudaMemsetAsync(ctx->scratch, 0, field_bytes(ctx), ctx->stream), "memset scratch");
+  fields_to_device(ctx, ctx->F.q, q);
+  refresh_traces(ctx, ctx->F);
+  ctx->t0 = t0; ctx->fine = 0;
+  sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+int dg_set_exterior(dg_ctx* ctx, const double* ext) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!ext) throw ApiError(DG_ERR_ARG, "ext is NULL");
+  upload_real(ctx, ctx->ext, ext, ctx->mesh.bnd_k.size() * ctx->Nfp * 2);
+  ctx->has_ext = true;
+  DG_CATCH(ctx)
+}
+
+}  // extern "C"

@@ -1,0 +1,352 @@
+// C ABI of libdgrtm, part 1: context, setup, device workspace (include/dgrtm.h).
+#include <algorithm>
+#include <cmath>
+#include <mutex>
+
+#include "ctx.h"
+
+namespace dgrtm {
+
+const KernelTable* dg_kernel_table_order1(int);
+const KernelTable* dg_kernel_table_order2(int);
+const KernelTable* dg_kernel_table_order3(int);
+const KernelTable* dg_kernel_table_order4(int);
+const KernelTable* dg_kernel_table_order5(int);
+const KernelTable* dg_kernel_table_order6(int);
+
+const KernelTable* get_kernel_table(int N, int precision) {
+  switch (N) {
+    case 1: return dg_kernel_table_order1(precision);
+    case 2: return dg_kernel_table_order2(precision);
+    case 3: return dg_kernel_table_order3(precision);
+    case 4: return dg_kernel_table_order4(precision);
+    case 5: return dg_kernel_table_order5(precision);
+    case 6: return dg_kernel_table_order6(precision);
+  }
+  return nullptr;
+}
+
+// ---- Adams-Bashforth weights by exact polynomial integration (long double, rounded once) ---------
+namespace {
+typedef std::vector<long double> Poly;   // ascending coefficients
+Poly pmul(const Poly& p, const Poly& q) {
+  Poly o(p.size() + q.size() - 1, 0.0L);
+  for (size_t i = 0; i < p.size(); ++i)
+    for (size_t j = 0; j < q.size(); ++j) o[i + j] += p[i] * q[j];
+  return o;
+}
+Poly pint(const Poly& p) {
+  Poly o(p.size() + 1, 0.0L);
+  for (size_t i = 0; i < p.size(); ++i) o[i + 1] = p[i] / (long double)(i + 1);
+  return o;
+}
+long double peval(const Poly& p, long double x) {
+  long double v = 0;
+  for (size_t i = p.size(); i-- > 0;) v = v * x + p[i];
+  return v;
+}
+// I_s = antiderivative of the Lagrange function l_s through the nodes 0, -1, .., -(order-1)
+std::vector<Poly> ab_antiderivatives(int order) {
+  std::vector<Poly> I;
+  for (int s = 0; s < order; ++s) {
+    Poly p(1, 1.0L);
+    for (int j = 0; j < order; ++j) {
+      if (j == s) continue;
+      const long double xs = -(long double)s, xj = -(long double)j;
+      p = pmul(p, Poly{-xj / (xs - xj), 1.0L / (xs - xj)});
+    }
+    I.push_back(pint(p));
+  }
+  return I;
+}
+}  // namespace
+
+const AbCoef& ab_coef(int order) {
+  static AbCoef tab[4];
+  static std::once_flag once;
+  std::call_once(once, [] {
+    for (int m = 1; m <= 3; ++m) {
+      AbCoef& c = tab[m];
+      std::memset(&c, 0, sizeof(c));
+      std::vector<Poly> I = ab_antiderivatives(m);
+      for (int s = 0; s < m; ++s) {
+        c.a[s] = (double)peval(I[s], 1.0L);                 // eq (18)
+        c.b[s] = (double)peval(I[s], 0.5L);                 // eq (19)
+        c.abar[s] = (double)peval(pint(I[s]), 1.0L);        // reading Q1(iii)
+        for (int t = 0; t < m; ++t) c.C[3 * s + t] = (double)peval(pint(pmul(I[s], I[t])), 1.0L);  // (24)
+      }
+    }
+    std::memset(&tab[0], 0, sizeof(AbCoef));
+  });
+  return tab[order < 0 ? 0 : (order > 3 ? 3 : order)];
+}
+
+void ab_partial(int order, double theta, double w[3]) {
+  w[0] = w[1] = w[2] = 0;
+  if (order < 1) return;
+  std::vector<Poly> I = ab_antiderivatives(order > 3 ? 3 : order);
+  for (size_t s = 0; s < I.size(); ++s) w[s] = (double)peval(I[s], (long double)theta);
+}
+
+double ricker(double t, double f0, double tp, double amp) {
+  const double pi = 3.14159265358979323846;
+  const double x = pi * f0 * (t - tp), a = x * x;
+  return amp * (1.0 - 2.0 * a) * std::exp(-a);
+}
+
+// ---- small device helpers ------------------------------------------------------------------------
+size_t field_bytes(const dg_ctx* c) { return (size_t)c->model.nslots * 4 * c->Np * c->rs; }
+size_t trace_bytes(const dg_ctx* c) { return (size_t)c->model.nslots * 4 * c->REC * c->rs; }
+
+void sync_stream(dg_ctx* c) { cuda_check(cudaStreamSynchronize(c->stream), "cudaStreamSynchronize"); }
+
+void upload_raw(dg_ctx* c, void* dst, const void* src, size_t bytes) {
+  if (!bytes) return;
+  cuda_check(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream), "cudaMemcpyAsync H2D");
+  sync_stream(c);
+}
+
+void upload_real(dg_ctx* c, void* dst, const double* src, size_t n) {
+  if (!n) return;
+  if (c->precision == 64) { upload_raw(c, dst, src, n * sizeof(double)); return; }
+  std::vector<float> tmp(n);
+  for (size_t i = 0; i < n; ++i) tmp[i] = (float)src[i];
+  upload_raw(c, dst, tmp.data(), n * sizeof(float));
+}
+
+void download_real(dg_ctx* c, double* dst, const void* src, size_t n) {
+  if (!n) return;
+  if (c->precision == 64) {
+    cuda_check(cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
+    sync_stream(c);
+    return;
+  }
+  std::vector<float> tmp(n);
+  cuda_check(cudaMemcpyAsync(tmp.data(), src, n * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
+  sync_stream(c);
+  for (size_t i = 0; i < n; ++i) dst[i] = (double)tmp[i];
+}
+
+void fields_to_device(dg_ctx* c, char* dq, const double* q) {
+  const int Np = c->Np;
+  const int64_t ns = c->model.nslots;
+  std::vector<double> tmp((size_t)ns * 4 * Np, 0.0);
+  for (int64_t s = 0; s < ns; ++s) {
+    const int64_t k = c->model.elem_of[s];
+    if (k < 0) continue;
+    const int64_t b = s >> 5, lane = s & 31;
+    for (int x = 0; x < 4 * Np; ++x) tmp[((size_t)b * 4 * Np + x) * 32 + lane] = q[(size_t)k * 4 * Np + x];
+  }
+  upload_real(c, dq, tmp.data(), tmp.size());
+}
+
+void fields_from_device(dg_ctx* c, double* q, const char* dq) {
+  const int Np = c->Np;
+  const int64_t ns = c->model.nslots;
+  std::vector<double> tmp((size_t)ns * 4 * Np);
+  download_real(c, tmp.data(), dq, tmp.size());
+  for (int64_t s = 0; s < ns; ++s) {
+    const int64_t k = c->model.elem_of[s];
+    if (k < 0) continue;
+    const int64_t b = s >> 5, lane = s & 31;
+    for (int x = 0; x < 4 * Np; ++x) q[(size_t)k * 4 * Np + x] = tmp[((size_t)b * 4 * Np + x) * 32 + lane];
+  }
+}
+
+void clear_field(dg_ctx* c, Field& F) {
+  cuda_check(cudaMemsetAsync(F.q, 0, field_bytes(c), c->stream), "memset q");
+  for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(F.hist[s], 0, field_bytes(c), c->stream), "memset hist");
+  cuda_check(cudaMemsetAsync(F.qf, 0, trace_bytes(c), c->stream), "memset qf");
+  F.reset_history();
+}
+
+void refresh_traces(dg_ctx* c, Field& F) {
+  // update kernel with zero weights: q unchanged, exposed traces rewritten (Alg. 4)
+  UpdateArgs u;
+  std::memset(&u, 0, sizeof(u));
+  u.q = F.q; u.qf = F.qf; u.h0 = F.hist[0]; u.h1 = F.hist[1]; u.h2 = F.hist[2];
+  u.geo = c->geo; u.wperm = c->wperm; u.blk0 = 0; u.nblk = (int)c->model.nblocks;
+  u.c0 = u.c1 = u.c2 = 0; u.ops = c->ops;
+  c->kt->update(u, c->stream);
+  c->launches++;
+}
+
+}  // namespace dgrtm
+
+using namespace dgrtm;
+
+static thread_local std::string g_create_error;
+
+extern "C" {
+
+const char* dg_version(void) { return "dgrtm 0.1 (sm_100a)"; }
+
+const char* dg_last_error(const dg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, const int32_t* EToV,
+                   const double* VX, const int8_t* face_bc, int default_bc) {
+  if (!out) { g_create_error = "out is NULL"; return DG_ERR_ARG; }
+  *out = nullptr;
+  if (!EToV || !VX || K <= 0 || Nv <= 0) { g_create_error = "NULL / empty mesh arrays"; return DG_ERR_ARG; }
+  if (N < 1 || N > 6) { g_create_error = "order N must be in 1..6"; return DG_ERR_UNSUPPORTED; }
+  if (precision != 32 && precision != 64) { g_create_error = "precision must be 32 or 64"; return DG_ERR_UNSUPPORTED; }
+  if (default_bc < 1 || default_bc > 4) { g_create_error = "default_bc must be 1..4"; return DG_ERR_ARG; }
+  if (K > (int64_t)500000000 / 4) { g_create_error = "too many elements for 32-bit face indices"; return DG_ERR_UNSUPPORTED; }
+  dg_ctx* c = nullptr;
+  try {
+    c = new dg_ctx();
+    c->N = N; c->precision = precision; c->rs = precision == 64 ? 8 : 4;
+    build_reference_element(N, c->re);
+    c->Np = c->re.Np; c->Nfp = c->re.Nfp; c->NF = 4 * c->Nfp; c->REC = 2 * c->Nfp;
+    int64_t bad = -1;
+    std::string msg = build_mesh(c->re, K, Nv, EToV, VX, face_bc, default_bc, c->mesh, &bad);
+    if (!msg.empty()) {
+      g_create_error = msg + " (element " + std::to_string(bad) + ")";
+      delete c;
+      return DG_ERR_MESH;
+    }
+    for (size_t i = 0; i < c->mesh.bc.size(); ++i)
+      if (c->mesh.bc[i] == DG_BC_PRESCRIBED) c->has_prescribed = true;
+    c->kt = get_kernel_table(N, precision);
+    for (int l = 0; l < kMaxLevels; ++l) { c->d_coarse[l] = nullptr; c->d_stored[l] = nullptr; c->rec[l] = nullptr; }
+    c->F.reset_history(); c->R.reset_history();
+  } catch (const std::exception& e) {
+    g_create_error = e.what();
+    delete c;
+    return DG_ERR_ARG;
+  }
+  *out = c;
+  return DG_OK;
+}
+
+void dg_destroy(dg_ctx* ctx) { delete ctx; }
+
+int dg_set_model(dg_ctx* ctx, const double* rho, const double* c, int nlevels, double cfl) {
+  DG_TRY(ctx)
+  if (!rho || !c) throw ApiError(DG_ERR_ARG, "rho / c is NULL");
+  if (nlevels < 1 || nlevels > kMaxLevels) throw ApiError(DG_ERR_UNSUPPORTED, "nlevels must be in 1..8");
+  if (!(cfl > 0)) throw ApiError(DG_ERR_ARG, "cfl must be positive");
+  for (int64_t k = 0; k < ctx->mesh.K; ++k)
+    if (!(rho[k] > 0) || !(c[k] > 0)) throw ApiError(DG_ERR_ARG, "rho and c must be positive (element " + std::to_string(k) + ")");
+  build_model(ctx->re, ctx->mesh, rho, c, nlevels, cfl, ctx->model);
+  ctx->dt_local = ctx->model.dt_local;
+  ctx->nlocal = 1 << (nlevels - 1);
+  ctx->has_model = true;
+  ctx->bound = false; ctx->hist_bound = false;     // the slot layout changed
+  DG_CATCH(ctx)
+}
+
+int dg_set_integrator(dg_ctx* ctx, int integrator) {
+  DG_TRY(ctx)
+  if (integrator != DG_INTEGRATOR_AB3 && integrator != DG_INTEGRATOR_LSERK4) throw ApiError(DG_ERR_ARG, "unknown integrator");
+  if (integrator == DG_INTEGRATOR_LSERK4 && ctx->has_model && ctx->model.nlevels != 1)
+    throw ApiError(DG_ERR_UNSUPPORTED, "LSERK4 is single-rate only");
+  ctx->integrator = integrator;
+  DG_CATCH(ctx)
+}
+
+int dg_set_dt(dg_ctx* ctx, double dt_local) {
+  DG_TRY(ctx)
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  if (!(dt_local > 0)) throw ApiError(DG_ERR_ARG, "dt_local must be positive");
+  ctx->dt_local = dt_local;
+  DG_CATCH(ctx)
+}
+
+static void point_weights(dg_ctx* c, const double x[3], int64_t* k, double* row, double* w) {
+  double rst[3];
+  const int64_t e = c->locator.locate(c->mesh, x, rst);
+  if (e < 0) throw ApiError(DG_ERR_ARG, "point outside the mesh");
+  const int Np = c->Np;
+  std::vector<double> ell(Np);
+  c->re.interp_row(rst[0], rst[1], rst[2], ell.data());
+  for (int n = 0; n < Np; ++n) {
+    double acc = 0;
+    for (int m = 0; m < Np; ++m) acc += c->re.Minv[(size_t)n * Np + m] * ell[m];
+    w[n] = acc / c->mesh.J[e];                      // M_k^-1 l(x0), M_k = J_k M
+    if (row) row[n] = ell[n];
+  }
+  *k = e;
+}
+
+int dg_set_source(dg_ctx* ctx, const double x0[3], int wavelet, double f0, double tp, double amp) {
+  DG_TRY(ctx)
+  if (!x0) throw ApiError(DG_ERR_ARG, "x0 is NULL");
+  if (wavelet != DG_WAVELET_RICKER) throw ApiError(DG_ERR_UNSUPPORTED, "unknown wavelet");
+  ctx->src_w.assign(ctx->Np, 0.0);
+  point_weights(ctx, x0, &ctx->src_k, nullptr, ctx->src_w.data());
+  ctx->f0 = f0; ctx->tp = tp; ctx->amp = amp;
+  ctx->has_src = true;
+  if (ctx->bound) upload_real(ctx, ctx->d_src_w, ctx->src_w.data(), ctx->Np);
+  DG_CATCH(ctx)
+}
+
+int dg_set_receivers(dg_ctx* ctx, int64_t nr, const double* xr) {
+  DG_TRY(ctx)
+  if (nr < 0 || (nr > 0 && !xr)) throw ApiError(DG_ERR_ARG, "bad receiver array");
+  const int Np = ctx->Np;
+  std::vector<int32_t> rk(nr);
+  std::vector<double> row((size_t)nr * Np), w((size_t)nr * Np);
+  for (int64_t r = 0; r < nr; ++r) {
+    int64_t k;
+    point_weights(ctx, xr + 3 * r, &k, &row[(size_t)r * Np], &w[(size_t)r * Np]);
+    rk[r] = (int32_t)k;
+  }
+  ctx->nr = nr; ctx->rcv_k.swap(rk); ctx->rcv_row.swap(row); ctx->rcv_w.swap(w);
+  ctx->hist_bound = false;
+  DG_CATCH(ctx)
+}
+
+// ---- workspace -------------------------------------------------------------------------------------
+} // extern C
+namespace dgrtm {
+void carve_workspace(dg_ctx* c, Carver& cv) {
+  const int Np = c->Np, Nfp = c->Nfp, NF = c->NF;
+  const size_t rs = c->rs;
+  const Model& md = c->model;
+  c->ops.D3T = cv.take((size_t)3 * Np * Np * rs);
+  c->ops.LIFTT = cv.take((size_t)NF * Np * rs);
+  c->ops.Fmask = (const int*)cv.take((size_t)NF * 4);
+  c->ops.nperm = (int)(c->mesh.ptab.size() / Nfp);
+  c->ops.ptab = (const int*)cv.take(c->mesh.ptab.size() * 4);
+  c->geo = cv.take((size_t)md.nblocks * DG_NGEO * 32 * rs);
+  c->nbr = (int*)cv.take((size_t)md.nblocks * 4 * 32 * 4);
+  c->wperm = (int*)cv.take((size_t)md.nblocks * 32 * 4);
+  c->F.q = cv.take(field_bytes(c));
+  for (int s = 0; s < 3; ++s) c->F.hist[s] = cv.take(field_bytes(c));
+  c->F.qf = cv.take(trace_bytes(c));
+  c->scratch = cv.take(field_bytes(c));
+  c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);
+  c->d_src_w = cv.take((size_t)Np * rs);
+  for (int l = 0; l < md.nlevels; ++l) {
+    c->d_coarse[l] = (int*)cv.take(std::max<size_t>(1, md.coarse_nb[l].size()) * 4);
+    c->d_stored[l] = (int*)cv.take(std::max<size_t>(1, md.stored[l].size()) * 4);
+  }
+}
+void require_bound(dg_ctx* c) {
+  if (!c->bound) throw ApiError(DG_ERR_STATE, "no device workspace bound (dg_set_model, dg_workspace_bytes, dg_bind_workspace)");
+}
+}  // namespace dgrtm
+extern "C" {
+
+int dg_workspace_bytes(dg_ctx* ctx, size_t* n) {
+  DG_TRY(ctx)
+  if (!n) throw ApiError(DG_ERR_ARG, "n is NULL");
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  Carver count;   // null base: only counts
+  {
+    // the carve writes pointers into the ctx: save and restore them so a bound ctx is not disturbed
+    OpsDev ops = ctx->ops; char* geo = ctx->geo; int* nbr = ctx->nbr; int* wperm = ctx->wperm; Field F = ctx->F;
+    char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w;
+    int* dc[kMaxLevels]; int* ds[kMaxLevels];
+    for (int l = 0; l < kMaxLevels; ++l) { dc[l] = ctx->d_coarse[l]; ds[l] = ctx->d_stored[l]; }
+    carve_workspace(ctx, count);
+    ctx->ops = ops; ctx->geo = geo; ctx->nbr = nbr; ctx->wperm = wperm; ctx->F = F;
+    ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw;
+    for (int l = 0; l < kMaxLevels; ++l) { ctx->d_coarse[l] = dc[l]; ctx->d_stored[l] = ds[l]; }
+  }
+  *n = count.used;
+  DG_CATCH(ctx)
+}
+
+}  // extern "C"

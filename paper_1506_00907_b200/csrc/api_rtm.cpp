@@ -1,0 +1,287 @@
+// C ABI of libdgrtm, part 4: reverse-time migration (Fig. 1): forward
+// phase with boundary-trace capture, backward phase with trace replay, receiver injection and the
+// imaging condition fused into the update.  All history stays in HBM (PAPER.md:407 kept it on the
+// host / HDD because a K20 could not hold it).
+#include <algorithm>
+#include <map>
+
+#include "ctx.h"
+
+using namespace dgrtm;
+
+namespace {
+
+int64_t records_of_level(const dg_ctx* c, int l, int nsteps) { return ((int64_t)nsteps << l) + 1; }
+
+void group_receivers(dg_ctx* c) {
+  const Model& md = c->model;
+  std::map<int64_t, std::vector<int32_t>> by_slot;
+  for (int64_t r = 0; r < c->nr; ++r) by_slot[md.slot_of[c->rcv_k[r]]].push_back((int32_t)r);
+  c->grp_slot.clear(); c->grp_off.assign(1, 0); c->grp_rcv.clear();
+  for (auto& kv : by_slot) {
+    c->grp_slot.push_back((int32_t)kv.first);
+    for (int32_t r : kv.second) c->grp_rcv.push_back(r);
+    c->grp_off.push_back((int32_t)c->grp_rcv.size());
+  }
+  // groups are ascending in slot, hence in level
+  size_t g = 0;
+  for (int l = 0; l <= md.nlevels; ++l) {
+    const int64_t first_slot = l < md.nlevels ? (int64_t)md.lvl_blk0[l] * 32 : md.nslots;
+    while (g < c->grp_slot.size() && c->grp_slot[g] < first_slot) ++g;
+    c->grp_lvl0[l] = (int)g;
+  }
+  for (int l = md.nlevels + 1; l <= kMaxLevels; ++l) c->grp_lvl0[l] = (int)c->grp_slot.size();
+}
+
+void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
+  const Model& md = c->model;
+  const size_t rs = c->rs;
+  const int Np = c->Np;
+  for (int l = 0; l < md.nlevels; ++l)
+    c->rec[l] = cv.take((size_t)records_of_level(c, l, nsteps) * md.stored[l].size() * c->REC * rs);
+  const size_t nr = (size_t)std::max<int64_t>(1, c->nr);
+  c->d_data = cv.take(nr * ((size_t)nsteps * c->nlocal + 1) * rs);
+  c->d_rcv_slot = (int*)cv.take(nr * 4);
+  c->d_rcv_level = (int*)cv.take(nr * 4);
+  c->d_rcv_row = cv.take(nr * Np * rs);
+  c->d_rcv_w = cv.take(nr * Np * rs);
+  c->d_grp_slot = (int*)cv.take(nr * 4);
+  c->d_grp_off = (int*)cv.take((nr + 1) * 4);
+  c->d_grp_rcv = (int*)cv.take(nr * 4);
+  c->R.q = cv.take(field_bytes(c));
+  for (int s = 0; s < 3; ++s) c->R.hist[s] = cv.take(field_bytes(c));
+  c->R.qf = cv.take(trace_bytes(c));
+  c->image = cv.take((size_t)md.nblocks * Np * 32 * rs);
+  c->qfinal = cv.take(field_bytes(c));
+}
+
+struct HistPtrs {   // everything carve_history writes, for save / restore around a size query
+  char* rec[kMaxLevels]; char* d_data; int* a; int* b; char* cc; char* d; int* e; int* f; int* g; Field R; char* image; char* qfinal;
+  void save(const dg_ctx* c) {
+    for (int l = 0; l < kMaxLevels; ++l) rec[l] = c->rec[l];
+    d_data = c->d_data; a = c->d_rcv_slot; b = c->d_rcv_level; cc = c->d_rcv_row; d = c->d_rcv_w;
+    e = c->d_grp_slot; f = c->d_grp_off; g = c->d_grp_rcv; R = c->R; image = c->image; qfinal = c->qfinal;
+  }
+  void restore(dg_ctx* c) const {
+    for (int l = 0; l < kMaxLevels; ++l) c->rec[l] = rec[l];
+    c->d_data = d_data; c->d_rcv_slot = a; c->d_rcv_level = b; c->d_rcv_row = cc; c->d_rcv_w = d;
+    c->d_grp_slot = e; c->d_grp_off = f; c->d_grp_rcv = g; c->R = R; c->image = image; c->qfinal = qfinal;
+  }
+};
+
+void require_history(dg_ctx* c) {
+  require_bound(c);
+  if (!c->hist_bound) throw ApiError(DG_ERR_STATE, "no RTM history bound (rtm_history_bytes, rtm_bind_history)");
+}
+
+// host [nr][ncol_host] <-> device [nr][nsamp] (leading columns)
+void copy_data(dg_ctx* c, double* host, const double* host_in, int64_t ncol) {
+  const int64_t nsamp = (int64_t)c->hist_nsteps * c->nlocal + 1;
+  const size_t rs = c->rs;
+  if (c->nr == 0) return;
+  if (host_in) {
+    std::vector<char> tmp((size_t)c->nr * ncol * rs);
+    for (size_t i = 0; i < (size_t)c->nr * ncol; ++i) {
+      if (c->precision == 64) ((double*)tmp.data())[i] = host_in[i];
+      else ((float*)tmp.data())[i] = (float)host_in[i];
+    }
+    cuda_check(cudaMemcpy2DAsync(c->d_data, nsamp * rs, tmp.data(), ncol * rs, ncol * rs, c->nr,
+                                 cudaMemcpyHostToDevice, c->stream), "cudaMemcpy2DAsync data H2D");
+    sync_stream(c);
+  } else {
+    std::vector<char> tmp((size_t)c->nr * ncol * rs);
+    cuda_check(cudaMemcpy2DAsync(tmp.data(), ncol * rs, c->d_data, nsamp * rs, ncol * rs, c->nr,
+                                 cudaMemcpyDeviceToHost, c->stream), "cudaMemcpy2DAsync data D2H");
+    sync_stream(c);
+    for (size_t i = 0; i < (size_t)c->nr * ncol; ++i)
+      host[i] = c->precision == 64 ? ((double*)tmp.data())[i] : (double)((float*)tmp.data())[i];
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n) {
+  DG_TRY(ctx)
+  if (!n) throw ApiError(DG_ERR_ARG, "n is NULL");
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  if (nsteps < 1) throw ApiError(DG_ERR_ARG, "nsteps must be >= 1");
+  HistPtrs keep;
+  keep.save(ctx);
+  Carver count;
+  carve_history(ctx, count, nsteps);
+  keep.restore(ctx);
+  *n = count.used;
+  DG_CATCH(ctx)
+}
+
+int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!dptr || ((uintptr_t)dptr & 255) != 0) throw ApiError(DG_ERR_ARG, "device pointer must be non-NULL and 256-byte aligned");
+  // the largest nsteps that fits decides the record capacity
+  int nsteps = 0;
+  {
+    HistPtrs keep;
+    keep.save(ctx);
+    int lo = 0, hi = 1;
+    auto fits = [&](int s) { Carver cnt; carve_history(ctx, cnt, s); return cnt.used <= n; };
+    if (fits(1)) {
+      lo = 1;
+      while (hi < (1 << 28) && fits(hi * 2)) hi *= 2;
+      lo = hi; hi = hi * 2;
+      while (hi - lo > 1) { const int mid = lo + (hi - lo) / 2; if (fits(mid)) lo = mid; else hi = mid; }
+    }
+    keep.restore(ctx);
+    nsteps = lo;
+  }
+  if (nsteps < 1) throw ApiError(DG_ERR_NOMEM, "history buffer too small for a single step");
+  ctx->hs = (char*)dptr; ctx->hs_bytes = n; ctx->hist_nsteps = nsteps;
+  Carver cv;
+  cv.base = ctx->hs;
+  carve_history(ctx, cv, nsteps);
+  // receiver tables
+  group_receivers(ctx);
+  const int64_t nr = ctx->nr;
+  if (nr) {
+    std::vector<int32_t> slot(nr), lvl(nr);
+    for (int64_t r = 0; r < nr; ++r) {
+      slot[r] = (int32_t)ctx->model.slot_of[ctx->rcv_k[r]];
+      lvl[r] = ctx->model.level[ctx->rcv_k[r]];
+    }
+    upload_raw(ctx, ctx->d_rcv_slot, slot.data(), nr * 4);
+    upload_raw(ctx, ctx->d_rcv_level, lvl.data(), nr * 4);
+    upload_real(ctx, ctx->d_rcv_row, ctx->rcv_row.data(), ctx->rcv_row.size());
+    upload_real(ctx, ctx->d_rcv_w, ctx->rcv_w.data(), ctx->rcv_w.size());
+    upload_raw(ctx, ctx->d_grp_slot, ctx->grp_slot.data(), ctx->grp_slot.size() * 4);
+    upload_raw(ctx, ctx->d_grp_off, ctx->grp_off.data(), ctx->grp_off.size() * 4);
+    upload_raw(ctx, ctx->d_grp_rcv, ctx->grp_rcv.data(), ctx->grp_rcv.size() * 4);
+  }
+  ctx->hist_bound = true;
+  clear_field(ctx, ctx->R);
+  cuda_check(cudaMemsetAsync(ctx->image, 0, (size_t)ctx->model.nblocks * ctx->Np * 32 * ctx->rs, ctx->stream), "memset image");
+  ctx->have_final = false; ctx->have_backward = false;
+  sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (nsteps < 1 || nsteps > ctx->hist_nsteps) throw ApiError(DG_ERR_NOMEM, "nsteps exceeds the bound history capacity (" + std::to_string(ctx->hist_nsteps) + ")");
+  if (ctx->integrator != DG_INTEGRATOR_AB3) throw ApiError(DG_ERR_UNSUPPORTED, "RTM uses the AB3 / multi-rate AB3 integrator");
+  clear_field(ctx, ctx->F);
+  ctx->t0 = 0; ctx->fine = 0;
+  RunOpts o;
+  o.direction = 1; o.fields[0] = &ctx->F; o.nfields = 1; o.source_on[0] = ctx->has_src;
+  o.capture = true; o.record = ctx->nr > 0; o.first_fine = 0; o.t0 = 0;
+  run_mrab(ctx, nsteps, o);
+  ctx->fine = (int64_t)nsteps * ctx->nlocal;
+  cuda_check(cudaMemcpyAsync(ctx->qfinal, ctx->F.q, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "save final state");
+  cuda_check(cudaGetLastError(), "kernel launch");
+  ctx->have_final = true; ctx->final_nsteps = nsteps; ctx->have_backward = false;
+  if (data_out) copy_data(ctx, data_out, nullptr, (int64_t)nsteps * ctx->nlocal + 1);
+  sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
+                      int64_t first_image_step) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (!ctx->have_final) throw ApiError(DG_ERR_STATE, "rtm_forward_shot first");
+  if (nsteps < 1 || nsteps > ctx->final_nsteps) throw ApiError(DG_ERR_ARG, "nsteps must be in 1..(steps of the forward shot)");
+  if (!updir) throw ApiError(DG_ERR_ARG, "updir is NULL");
+  if (imaging != DG_IMAGING_CLASSICAL && imaging != DG_IMAGING_CHARACTERISTIC) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
+  const int64_t ntot = ctx->final_nsteps;
+  if (data) copy_data(ctx, nullptr, data, ntot * ctx->nlocal + 1);   // NULL: the signals recorded on the device
+  // source field: restart from q(t_f) (history restarts, reading Q7); receiver field: from rest
+  cuda_check(cudaMemcpyAsync(ctx->F.q, ctx->qfinal, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "restore final state");
+  for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(ctx->F.hist[s], 0, field_bytes(ctx), ctx->stream), "memset hist");
+  ctx->F.reset_history();
+  refresh_traces(ctx, ctx->F);
+  clear_field(ctx, ctx->R);
+  RunOpts o;
+  o.direction = -1; o.fields[0] = &ctx->F; o.fields[1] = &ctx->R; o.nfields = 2;
+  o.source_on[0] = ctx->has_src; o.source_on[1] = false;
+  o.replay = true; o.inject_field = ctx->nr > 0 ? 1 : -1;
+  o.image = true; o.imaging = imaging;
+  for (int d = 0; d < 3; ++d) o.updir[d] = updir[d];
+  o.image_min_fine = first_image_step * ctx->nlocal;
+  o.first_fine = ntot * ctx->nlocal;
+  o.t0 = (double)ntot * ((double)ctx->nlocal * ctx->dt_local);
+  run_mrab(ctx, nsteps, o);
+  ctx->fine = (ntot - nsteps) * ctx->nlocal;
+  cuda_check(cudaGetLastError(), "kernel launch");
+  ctx->have_backward = true;
+  sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+int rtm_image_read(dg_ctx* ctx, double* I_out) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (!I_out) throw ApiError(DG_ERR_ARG, "I_out is NULL");
+  const int Np = ctx->Np;
+  std::vector<double> tmp((size_t)ctx->model.nblocks * Np * 32);
+  download_real(ctx, tmp.data(), ctx->image, tmp.size());
+  for (int64_t s = 0; s < ctx->model.nslots; ++s) {
+    const int64_t k = ctx->model.elem_of[s];
+    if (k < 0) continue;
+    for (int n = 0; n < Np; ++n) I_out[(size_t)k * Np + n] = tmp[(((size_t)(s >> 5)) * Np + n) * 32 + (s & 31)];
+  }
+  DG_CATCH(ctx)
+}
+
+int rtm_image_zero(dg_ctx* ctx) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  cuda_check(cudaMemsetAsync(ctx->image, 0, (size_t)ctx->model.nblocks * ctx->Np * 32 * ctx->rs, ctx->stream), "memset image");
+  DG_CATCH(ctx)
+}
+
+int rtm_get_trace_index(const dg_ctx* ctx, int level, int64_t* nfaces, int64_t* nrecords, int32_t* faces) {
+  if (!ctx) return DG_ERR_ARG;
+  if (!ctx->has_model || level < 0 || level >= ctx->model.nlevels) return DG_ERR_ARG;
+  const std::vector<int32_t>& st = ctx->model.stored[level];
+  if (nfaces) *nfaces = (int64_t)st.size();
+  if (nrecords) *nrecords = ctx->hist_bound ? records_of_level(ctx, level, ctx->have_final ? ctx->final_nsteps : ctx->hist_nsteps) : 0;
+  if (faces) std::copy(st.begin(), st.end(), faces);
+  return DG_OK;
+}
+
+int rtm_get_traces(dg_ctx* ctx, int level, int64_t record, double* buf) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (!buf || level < 0 || level >= ctx->model.nlevels) throw ApiError(DG_ERR_ARG, "bad level / buffer");
+  if (record < 0 || record >= records_of_level(ctx, level, ctx->hist_nsteps)) throw ApiError(DG_ERR_ARG, "record out of range");
+  const size_t nf = ctx->model.stored[level].size(), Nfp = ctx->Nfp;
+  std::vector<double> tmp(nf * 2 * Nfp);
+  download_real(ctx, tmp.data(), ctx->rec[level] + (size_t)record * nf * ctx->REC * ctx->rs, tmp.size());
+  // device record: [face][p | n.v][Nfp]  ->  buf[face][Nfp][2]
+  for (size_t x = 0; x < nf; ++x)
+    for (size_t i = 0; i < Nfp; ++i) {
+      buf[(x * Nfp + i) * 2 + 0] = tmp[x * 2 * Nfp + i];
+      buf[(x * Nfp + i) * 2 + 1] = tmp[x * 2 * Nfp + Nfp + i];
+    }
+  DG_CATCH(ctx)
+}
+
+int rtm_get_fields(dg_ctx* ctx, int which, double* q) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (!q) throw ApiError(DG_ERR_ARG, "q is NULL");
+  if (which == 0) {
+    if (!ctx->have_final) throw ApiError(DG_ERR_STATE, "rtm_forward_shot first");
+    fields_from_device(ctx, q, ctx->qfinal);
+  } else if (which == 1 || which == 2) {
+    if (!ctx->have_backward) throw ApiError(DG_ERR_STATE, "rtm_backward_shot first");
+    fields_from_device(ctx, q, which == 1 ? ctx->F.q : ctx->R.q);
+  } else {
+    throw ApiError(DG_ERR_ARG, "which must be 0, 1 or 2");
+  }
+  DG_CATCH(ctx)
+}
+
+}  // extern "C"

@@ -1,0 +1,311 @@
+// C ABI of libdgrtm, part 3: the time-stepping schedule of Algorithm 1 on the
+// device kernels, forward or backward in time, one or two wavefields.
+#include <algorithm>
+#include <cmath>
+
+#include "ctx.h"
+
+namespace dgrtm {
+
+namespace {
+
+inline int lvl_blk_end(const Model& md, int l) { return md.lvl_blk0[l] + md.lvl_nblk[l]; }
+
+void launch_update(dg_ctx* c, Field& F, int l, double dts) {
+  const AbCoef& co = ab_coef(F.nhist[l]);
+  UpdateArgs u;
+  std::memset(&u, 0, sizeof(u));
+  u.q = F.q; u.qf = F.qf; u.h0 = F.h(l, 0); u.h1 = F.h(l, 1); u.h2 = F.h(l, 2);
+  u.geo = c->geo; u.wperm = c->wperm;
+  u.blk0 = c->model.lvl_blk0[l]; u.nblk = c->model.lvl_nblk[l];
+  u.c0 = dts * co.a[0]; u.c1 = dts * co.a[1]; u.c2 = dts * co.a[2];      // eq (18)
+  u.ops = c->ops;
+  if (u.nblk > 0) { c->kt->update(u, c->stream); c->launches++; }
+}
+
+void launch_half(dg_ctx* c, Field& F, int l, double dts) {
+  const int n = (int)c->model.coarse_nb[l].size();
+  if (!n) return;
+  const AbCoef& co = ab_coef(F.nhist[l]);
+  HalfArgs h;
+  std::memset(&h, 0, sizeof(h));
+  h.q = F.q; h.qf = F.qf; h.h0 = F.h(l, 0); h.h1 = F.h(l, 1); h.h2 = F.h(l, 2);
+  h.geo = c->geo; h.wperm = c->wperm; h.list = c->d_coarse[l]; h.nlist = n;
+  h.c0 = dts * co.b[0]; h.c1 = dts * co.b[1]; h.c2 = dts * co.b[2];      // eq (19)
+  h.ops = c->ops;
+  c->kt->half(h, c->stream);
+  c->launches++;
+}
+
+void launch_image_update(dg_ctx* c, Field& S, Field& R, int l, double dts, const RunOpts& o) {
+  const AbCoef& co = ab_coef(S.nhist[l]);
+  ImageArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.qS = S.q; a.qfS = S.qf; a.hS0 = S.h(l, 0); a.hS1 = S.h(l, 1); a.hS2 = S.h(l, 2);
+  a.qR = R.q; a.qfR = R.qf; a.hR0 = R.h(l, 0); a.hR1 = R.h(l, 1); a.hR2 = R.h(l, 2);
+  a.image = c->image; a.geo = c->geo; a.wperm = c->wperm;
+  a.blk0 = c->model.lvl_blk0[l]; a.nblk = c->model.lvl_nblk[l];
+  a.dts = dts;
+  for (int s = 0; s < 3; ++s) { a.a[s] = co.a[s]; a.abar[s] = co.abar[s]; }
+  for (int s = 0; s < 9; ++s) a.C[s] = co.C[s];
+  for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
+  a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
+  a.ops = c->ops;
+  if (a.nblk > 0) { c->kt->image_update(a, c->stream); c->launches++; }
+}
+
+PointArgs point_args(dg_ctx* c, const Field& F) {
+  PointArgs p;
+  std::memset(&p, 0, sizeof(p));
+  p.q = F.q;
+  for (int s = 0; s < 3; ++s) p.hist[s] = F.hist[s];
+  for (int l = 0; l < kMaxLevels; ++l) p.cur[l] = F.cur[l];
+  return p;
+}
+
+}  // namespace
+
+// right-hand side of levels l0..l1-1 of field F into `out` (a full-size [nslots][4Np] array)
+void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double dir, char* capture,
+                const char* replay) {
+  const Model& md = c->model;
+  RhsArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.q = F.q; a.qf = F.qf; a.rhs = out; a.geo = c->geo; a.nbr = c->nbr;
+  a.blk0 = md.lvl_blk0[l0]; a.nblk = lvl_blk_end(md, l1 - 1) - a.blk0;
+  a.mode = mode; a.dir = dir; a.capture = capture; a.replay = replay;
+  a.ext = c->has_ext ? c->ext : nullptr;
+  a.ops = c->ops;
+  if (a.nblk > 0) { c->kt->rhs(a, c->stream); c->launches++; }
+}
+
+void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
+  const Model& md = c->model;
+  const int L = md.nlevels, nloc = c->nlocal, dir = o.direction;
+  const double dtl = c->dt_local;
+  if (c->has_prescribed && !c->has_ext) throw ApiError(DG_ERR_STATE, "prescribed-exterior faces need dg_set_exterior");
+  int stride[kMaxLevels];
+  for (int l = 0; l < L; ++l) stride[l] = 1 << (L - 1 - l);
+  const int src_level = c->has_src ? md.level[c->src_k] : -1;
+  const int64_t nsamp = (int64_t)c->hist_nsteps * nloc + 1;
+  auto record_ptr = [&](int l, int64_t j) -> char* {
+    return c->rec[l] + (size_t)j * md.stored[l].size() * c->REC * c->rs;
+  };
+  auto sample_receivers = [&](int64_t m, int64_t jabs) {
+    PointArgs p = point_args(c, *o.fields[0]);
+    p.nr = (int)c->nr; p.rcv_slot = c->d_rcv_slot; p.rcv_row = c->d_rcv_row; p.rcv_level = c->d_rcv_level;
+    p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
+    for (int l = 0; l < L; ++l) {
+      const int off = (int)(m % stride[l]);
+      double w[3] = {0, 0, 0};
+      if (off) ab_partial(o.fields[0]->nhist[l], (double)off / stride[l], w);   // reading Q13
+      for (int s = 0; s < 3; ++s) p.lw[l][s] = dir * stride[l] * dtl * w[s];
+    }
+    c->kt->record(p, c->stream);
+    c->launches++;
+  };
+
+  const int64_t nfine = (int64_t)nglobal * nloc;
+  for (int64_t m = 0; m < nfine; ++m) {
+    const int64_t jabs = o.first_fine + dir * m;
+    const double t_start = o.t0 + dir * (double)m * dtl;
+    // ---- right-hand sides of every level whose unknowns sit at t_start
+    for (int l = 0; l < L; ++l) {
+      if (m % stride[l] != 0 || md.lvl_nblk[l] == 0) continue;
+      for (int fi = 0; fi < o.nfields; ++fi) {
+        Field& F = *o.fields[fi];
+        F.cur[l] = (F.cur[l] + 1) % 3;
+        char* out = F.hist[F.cur[l]];
+        char* cap = (fi == 0 && o.capture && !md.stored[l].empty()) ? record_ptr(l, jabs / stride[l]) : nullptr;
+        const char* rep = (fi == 0 && o.replay && !md.stored[l].empty()) ? record_ptr(l, jabs / stride[l]) : nullptr;
+        launch_rhs(c, F, out, l, l + 1, RHS_VOL | RHS_SURF, (double)dir, cap, rep);
+        if (o.source_on[fi] && src_level == l) {                       // eq (15), reading Q5
+          PointArgs p = point_args(c, F);
+          p.rhs = out; p.src_slot = (int)md.slot_of[c->src_k]; p.src_w = c->d_src_w;
+          p.amp_now = ricker(t_start, c->f0, c->tp, c->amp);
+          c->kt->source(p, c->stream);
+          c->launches++;
+        }
+        if (o.inject_field == fi && c->grp_lvl0[l + 1] > c->grp_lvl0[l]) {
+          PointArgs p = point_args(c, F);
+          p.rhs = out; p.rcv_w = c->d_rcv_w; p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
+          p.g0 = c->grp_lvl0[l]; p.ng = c->grp_lvl0[l + 1] - c->grp_lvl0[l];
+          p.grp_slot = c->d_grp_slot; p.grp_off = c->d_grp_off; p.grp_rcv = c->d_grp_rcv;
+          c->kt->inject(p, c->stream);
+          c->launches++;
+        }
+        F.nhist[l] = std::min(F.nhist[l] + 1, 3);
+      }
+    }
+    if (o.record && c->nr > 0) sample_receivers(m, jabs);
+    // ---- updates (18) of the levels that land on t_new, finest first
+    int coarsest_updated = L;
+    for (int l = L - 1; l >= 0; --l) {
+      if ((m + 1) % stride[l] != 0) continue;
+      coarsest_updated = l;
+      if (md.lvl_nblk[l] == 0) continue;
+      const double dts = dir * (double)stride[l] * dtl;
+      const int64_t jend = jabs + dir * 1;     // fine index after this fine step
+      const bool img = o.image && std::min(jabs, jend) >= o.image_min_fine;
+      if (img) {
+        launch_image_update(c, *o.fields[0], *o.fields[1], l, dts, o);
+      } else {
+        for (int fi = 0; fi < o.nfields; ++fi) launch_update(c, *o.fields[fi], l, dts);
+      }
+    }
+    // ---- coarse neighbours that were not updated: half-step traces (19)
+    const int lc = coarsest_updated - 1;
+    if (lc >= 0 && lc < L) {
+      const double dts = dir * (double)stride[lc] * dtl;
+      for (int fi = 0; fi < o.nfields; ++fi) launch_half(c, *o.fields[fi], lc, dts);
+    }
+  }
+  const int64_t jend = o.first_fine + dir * nfine;
+  if (o.capture) {
+    for (int l = 0; l < L; ++l) {
+      if (md.stored[l].empty()) continue;
+      CaptureArgs a;
+      std::memset(&a, 0, sizeof(a));
+      a.q = o.fields[0]->q; a.geo = c->geo; a.faces = c->d_stored[l]; a.nfaces = (int)md.stored[l].size();
+      a.record = record_ptr(l, jend / stride[l]); a.ops = c->ops;
+      c->kt->capture(a, c->stream);
+      c->launches++;
+    }
+  }
+  if (o.record && c->nr > 0) sample_receivers(0, jend);
+}
+
+// five-stage LSERK4 of Carpenter & Kennedy (not in the paper; BASELINE.json config 1, reading Q8)
+void run_lserk4(dg_ctx* c, int nsteps) {
+  static const double A[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                              -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+  static const double B[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                              1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                              2277821191437.0 / 14882151754819.0};
+  static const double C[5] = {0.0, 1432997174477.0 / 9575080441755.0, 2526269341429.0 / 6820363962896.0,
+                              2006345519317.0 / 3224310063776.0, 2802321613138.0 / 2924317926251.0};
+  const Model& md = c->model;
+  if (md.nlevels != 1) throw ApiError(DG_ERR_UNSUPPORTED, "LSERK4 is single-rate only");
+  if (c->has_prescribed && !c->has_ext) throw ApiError(DG_ERR_STATE, "prescribed-exterior faces need dg_set_exterior");
+  Field& F = c->F;
+  const double dt = c->dt_local;
+  for (int n = 0; n < nsteps; ++n) {
+    const double t = c->t0 + (double)(c->fine + n) * dt;
+    for (int st = 0; st < 5; ++st) {
+      char* r = F.hist[0];
+      launch_rhs(c, F, r, 0, 1, RHS_VOL | RHS_SURF, 1.0, nullptr, nullptr);
+      if (c->has_src) {
+        PointArgs p;
+        std::memset(&p, 0, sizeof(p));
+        p.rhs = r; p.src_slot = (int)md.slot_of[c->src_k]; p.src_w = c->d_src_w;
+        p.amp_now = ricker(t + C[st] * dt, c->f0, c->tp, c->amp);
+        c->kt->source(p, c->stream);
+        c->launches++;
+      }
+      RkArgs k;
+      std::memset(&k, 0, sizeof(k));
+      k.q = F.q; k.qf = F.qf; k.res = c->scratch; k.r = r; k.geo = c->geo; k.wperm = c->wperm;
+      k.blk0 = 0; k.nblk = (int)md.nblocks; k.A = A[st]; k.B = B[st]; k.dt = dt; k.ops = c->ops;
+      c->kt->rk(k, c->stream);
+      c->launches++;
+    }
+  }
+}
+
+}  // namespace dgrtm
+
+using namespace dgrtm;
+
+extern "C" {
+
+int dg_step(dg_ctx* ctx, int nsteps) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (nsteps < 0) throw ApiError(DG_ERR_ARG, "nsteps must be >= 0");
+  if (ctx->integrator == DG_INTEGRATOR_LSERK4) {
+    run_lserk4(ctx, nsteps);
+    ctx->fine += nsteps;
+  } else {
+    RunOpts o;
+    o.direction = 1; o.fields[0] = &ctx->F; o.nfields = 1; o.source_on[0] = ctx->has_src;
+    o.first_fine = ctx->fine; o.t0 = ctx->t0 + (double)ctx->fine * ctx->dt_local;
+    run_mrab(ctx, nsteps, o);
+    ctx->fine += (int64_t)nsteps * ctx->nlocal;
+  }
+  cuda_check(cudaGetLastError(), "kernel launch");
+  DG_CATCH(ctx)
+}
+
+int dg_get_rhs(dg_ctx* ctx, int which, int direction, double* r) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!r) throw ApiError(DG_ERR_ARG, "r is NULL");
+  if (direction != 1 && direction != -1) throw ApiError(DG_ERR_ARG, "direction must be +1 or -1");
+  if (ctx->has_prescribed && !ctx->has_ext) throw ApiError(DG_ERR_STATE, "prescribed-exterior faces need dg_set_exterior");
+  int mode;
+  switch (which) {
+    case DG_RHS_VOLUME: mode = RHS_VOL; break;
+    case DG_RHS_SURFACE: mode = RHS_SURF; break;
+    case DG_RHS_TOTAL: mode = RHS_VOL | RHS_SURF; break;
+    default: throw ApiError(DG_ERR_ARG, "which must be DG_RHS_VOLUME, DG_RHS_SURFACE or DG_RHS_TOTAL");
+  }
+  // the scratch array doubles as the LSERK4 residual, which is dead between steps (A_1 = 0)
+  cuda_check(cudaMemsetAsync(ctx->scratch, 0, field_bytes(ctx), ctx->stream), "memset scratch");
+  launch_rhs(ctx, ctx->F, ctx->scratch, 0, ctx->model.nlevels, mode, (double)direction, nullptr, nullptr);
+  cuda_check(cudaGetLastError(), "kernel launch");
+  fields_from_device(ctx, r, ctx->scratch);
+  DG_CATCH(ctx)
+}
+
+int dg_get_launch_count(const dg_ctx* ctx, int64_t* n) {
+  if (!ctx || !n) return DG_ERR_ARG;
+  *n = ctx->launches;
+  return DG_OK;
+}
+
+int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (reps < 0) throw ApiError(DG_ERR_ARG, "reps must be >= 0");
+  const Model& md = ctx->model;
+  Field& F = ctx->F;
+  for (int i = 0; i < reps; ++i) {
+    switch (which) {
+      case 0: launch_rhs(ctx, F, F.hist[0], 0, md.nlevels, RHS_VOL, 1.0, nullptr, nullptr); break;
+      case 1: launch_rhs(ctx, F, F.hist[0], 0, md.nlevels, RHS_SURF, 1.0, nullptr, nullptr); break;
+      case 2: launch_rhs(ctx, F, F.hist[0], 0, md.nlevels, RHS_VOL | RHS_SURF, 1.0, nullptr, nullptr); break;
+      case 3: {
+        UpdateArgs u;
+        std::memset(&u, 0, sizeof(u));
+        u.q = F.q; u.qf = F.qf; u.h0 = F.hist[0]; u.h1 = F.hist[1]; u.h2 = F.hist[2];
+        u.geo = ctx->geo; u.wperm = ctx->wperm; u.blk0 = 0; u.nblk = (int)md.nblocks;
+        u.c0 = 1e-30; u.c1 = -1e-30; u.c2 = 1e-30; u.ops = ctx->ops;
+        ctx->kt->update(u, ctx->stream);
+        ctx->launches++;
+        break;
+      }
+      case 4: {
+        if (!ctx->hist_bound) throw ApiError(DG_ERR_STATE, "rtm_bind_history first");
+        ImageArgs a;
+        std::memset(&a, 0, sizeof(a));
+        Field& R = ctx->R;
+        a.qS = F.q; a.qfS = F.qf; a.hS0 = F.hist[0]; a.hS1 = F.hist[1]; a.hS2 = F.hist[2];
+        a.qR = R.q; a.qfR = R.qf; a.hR0 = R.hist[0]; a.hR1 = R.hist[1]; a.hR2 = R.hist[2];
+        a.image = ctx->image; a.geo = ctx->geo; a.wperm = ctx->wperm; a.blk0 = 0; a.nblk = (int)md.nblocks;
+        a.dts = -1e-30;
+        const AbCoef& co = ab_coef(3);
+        for (int s = 0; s < 3; ++s) { a.a[s] = co.a[s]; a.abar[s] = co.abar[s]; }
+        for (int s = 0; s < 9; ++s) a.C[s] = co.C[s];
+        a.e[2] = -1; a.characteristic = 1; a.ops = ctx->ops;
+        ctx->kt->image_update(a, ctx->stream);
+        ctx->launches++;
+        break;
+      }
+      default: throw ApiError(DG_ERR_ARG, "which must be 0..4");
+    }
+  }
+  cuda_check(cudaGetLastError(), "kernel launch");
+  DG_CATCH(ctx)
+}
+
+}  // extern "C"

@@ -1,0 +1,179 @@
+// Host runtime state behind the opaque dg_ctx handle of include/dgrtm.h.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstring>
+#include <stdexcept>
+#include <string>
+#include <vector>
+
+#include "../../include/dgrtm.h"
+#include "kernels.h"
+#include "mesh_setup.h"
+#include "refelem.h"
+
+namespace dgrtm {
+
+constexpr int kMaxLevels = 8;
+
+struct ApiError : std::runtime_error {
+  int code;
+  ApiError(int c, const std::string& m) : std::runtime_error(m), code(c) {}
+};
+
+inline void cuda_check(cudaError_t e, const char* what) {
+  if (e != cudaSuccess) throw ApiError(DG_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// One wavefield on the device: nodal values, the three most recent own right-hand sides (rotating
+// buffers, never the physical shift of PAPER.md:344) and the exposed traces.
+struct Field {
+  char* q = nullptr;
+  char* hist[3] = {nullptr, nullptr, nullptr};
+  char* qf = nullptr;
+  int cur[kMaxLevels];     // per level: which of hist[] holds the newest right-hand side
+  int nhist[kMaxLevels];   // per level: number of valid history entries (start-up order, reading Q7)
+  void reset_history() {
+    for (int l = 0; l < kMaxLevels; ++l) { cur[l] = 0; nhist[l] = 0; }
+  }
+  const char* h(int l, int s) const { return hist[(cur[l] + 3 - s) % 3]; }   // s = 0 newest
+};
+
+// carves 256-byte aligned regions out of a caller-owned device buffer
+struct Carver {
+  char* base = nullptr;
+  size_t used = 0;
+  char* take(size_t bytes) {
+    char* p = base ? base + used : nullptr;
+    used += (bytes + 255) & ~(size_t)255;
+    return p;
+  }
+};
+
+// Adams-Bashforth weights of order 1..3 (eqs (18), (19), (22)-(24); readings Q1, Q7)
+struct AbCoef {
+  double a[3], b[3], abar[3], C[9];
+};
+const AbCoef& ab_coef(int order);
+// I_s(theta) = int_0^theta l_s for the order-`order` interpolant (22)
+void ab_partial(int order, double theta, double w[3]);
+double ricker(double t, double f0, double tp, double amp);
+
+}  // namespace dgrtm
+
+#define DG_TRY(ctx) \
+  if (!(ctx)) return DG_ERR_ARG; \
+  try {
+#define DG_CATCH(ctx) \
+  } catch (const dgrtm::ApiError& e) { (ctx)->err = e.what(); return e.code; \
+  } catch (const std::bad_alloc&) { (ctx)->err = "out of host memory"; return DG_ERR_NOMEM; \
+  } catch (const std::exception& e) { (ctx)->err = e.what(); return DG_ERR_ARG; } \
+  return DG_OK;
+
+struct dg_ctx {
+  std::string err;
+  int N = 0, precision = 0, Np = 0, Nfp = 0, NF = 0, REC = 0;
+  size_t rs = 4;                            // sizeof(real)
+  dgrtm::RefElem re;
+  dgrtm::Mesh mesh;
+  dgrtm::Model model;
+  dgrtm::Locator locator;
+  const dgrtm::KernelTable* kt = nullptr;
+  bool has_model = false;
+  int integrator = DG_INTEGRATOR_AB3;
+  double dt_local = 0;
+  int nlocal = 1;                           // fine steps per global step
+  bool has_prescribed = false;
+
+  // point source (eq (15))
+  bool has_src = false;
+  int64_t src_k = -1;
+  std::vector<double> src_w;
+  double f0 = 0, tp = 0, amp = 0;
+  // receivers
+  int64_t nr = 0;
+  std::vector<int32_t> rcv_k;
+  std::vector<double> rcv_row, rcv_w;
+  std::vector<int32_t> grp_slot, grp_off, grp_rcv;   // receivers grouped by element, groups by level
+  int grp_lvl0[dgrtm::kMaxLevels + 1];
+
+  // ---- forward workspace
+  bool bound = false;
+  char* ws = nullptr;
+  size_t ws_bytes = 0;
+  cudaStream_t stream = nullptr;
+  dgrtm::OpsDev ops;
+  char* geo = nullptr;
+  int* nbr = nullptr;
+  int* wperm = nullptr;
+  dgrtm::Field F;
+  char* scratch = nullptr;                  // LSERK4 residual / dg_get_rhs output
+  char* ext = nullptr;                      // prescribed exterior states [nbnd][Nfp][2]
+  bool has_ext = false;
+  char* d_src_w = nullptr;
+  int* d_coarse[dgrtm::kMaxLevels];         // per level: slots with a finer face neighbour
+  int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
+  double t0 = 0;
+  int64_t fine = 0;                         // time = t0 + fine * dt_local
+
+  // ---- RTM region
+  bool hist_bound = false;
+  int hist_nsteps = 0;
+  char* hs = nullptr;
+  size_t hs_bytes = 0;
+  char* rec[dgrtm::kMaxLevels];             // per level: trace records [nrec][nfaces][2][Nfp]
+  char* d_data = nullptr;                   // [nr][nfine+1] recorded / injected signals
+  int* d_rcv_slot = nullptr;
+  int* d_rcv_level = nullptr;
+  char* d_rcv_row = nullptr;
+  char* d_rcv_w = nullptr;
+  int* d_grp_slot = nullptr;
+  int* d_grp_off = nullptr;
+  int* d_grp_rcv = nullptr;
+  dgrtm::Field R;                           // receiver wavefield of the backward phase
+  char* image = nullptr;
+  char* qfinal = nullptr;
+  bool have_final = false, have_backward = false;
+  int final_nsteps = 0;
+
+  int64_t launches = 0;
+};
+
+namespace dgrtm {
+
+// ---- helpers shared by the api_*.cpp files
+size_t field_bytes(const dg_ctx* c);        // one [nslots][4Np] array
+size_t trace_bytes(const dg_ctx* c);        // one qf array
+void upload_real(dg_ctx* c, void* dst, const double* src, size_t n);
+void download_real(dg_ctx* c, double* dst, const void* src, size_t n);
+void upload_raw(dg_ctx* c, void* dst, const void* src, size_t bytes);
+void sync_stream(dg_ctx* c);
+// user order q[K][4][Np]  <->  device [block][4Np][32]
+void fields_to_device(dg_ctx* c, char* dq, const double* q);
+void fields_from_device(dg_ctx* c, double* q, const char* dq);
+void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
+void clear_field(dg_ctx* c, Field& F);
+
+struct RunOpts {
+  int direction = 1;
+  Field* fields[2] = {nullptr, nullptr};
+  int nfields = 1;
+  bool source_on[2] = {false, false};
+  bool capture = false, replay = false, record = false;
+  int inject_field = -1;
+  bool image = false;
+  int imaging = DG_IMAGING_CHARACTERISTIC;
+  double updir[3] = {0, 0, -1};
+  int64_t image_min_fine = 0;               // steps whose end index (forward numbering) is below do not image
+  int64_t first_fine = 0;                   // absolute fine index of the start time, forward numbering
+  double t0 = 0;                            // start time
+};
+void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o);
+void run_lserk4(dg_ctx* c, int nsteps);
+void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double dir, char* capture,
+                const char* replay);
+void carve_workspace(dg_ctx* c, Carver& cv);
+void require_bound(dg_ctx* c);
+
+}  // namespace dgrtm

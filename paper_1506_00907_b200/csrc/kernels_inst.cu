@@ -1,0 +1,110 @@
+// One translation unit per order: compiled six times with -DDG_ORDER=1..6 (float and double each).
+#include "kernels.cuh"
+
+#ifndef DG_ORDER
+#error "compile with -DDG_ORDER=<1..6>"
+#endif
+
+namespace dgrtm {
+namespace {
+
+constexpr int N = DG_ORDER;
+constexpr int kSMs = 148;   // B200
+
+template <typename F> int blocks_per_sm(F kernel, int threads, size_t smem) {
+  int n = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kernel, threads, smem);
+  return n < 1 ? 1 : n;
+}
+
+inline int persistent_grid(int nblk, int per_sm) {
+  const int cap = kSMs * per_sm;
+  return nblk < cap ? nblk : cap;
+}
+
+template <typename real> struct Launch {
+  static int occ_rhs, occ_upd, occ_rk, occ_img;
+
+  static int init() {
+    cudaError_t e;
+    e = cudaFuncSetAttribute(k_rhs<real, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RhsSmem<real, N>::bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_update<real, N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)UpdSmem<N>::template bytes<real>(1));
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_update<real, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)UpdSmem<N>::template bytes<real>(1));
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_image_update<real, N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)UpdSmem<N>::template bytes<real>(2));
+    if (e != cudaSuccess) return (int)e;
+    const int th = 32 * Tiling<N>::T;
+    occ_rhs = blocks_per_sm(k_rhs<real, N>, th, RhsSmem<real, N>::bytes);
+    occ_upd = blocks_per_sm(k_update<real, N, 0>, th, UpdSmem<N>::template bytes<real>(1));
+    occ_rk = blocks_per_sm(k_update<real, N, 1>, th, UpdSmem<N>::template bytes<real>(1));
+    occ_img = blocks_per_sm(k_image_update<real, N>, th, UpdSmem<N>::template bytes<real>(2));
+    return 0;
+  }
+  static void rhs(const RhsArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    k_rhs<real, N><<<persistent_grid(a.nblk, occ_rhs), 32 * Tiling<N>::T, RhsSmem<real, N>::bytes, s>>>(a);
+  }
+  static void update(const UpdateArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    k_update<real, N, 0><<<persistent_grid(a.nblk, occ_upd), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(1), s>>>(a, RkArgs());
+  }
+  static void rk(const RkArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    k_update<real, N, 1><<<persistent_grid(a.nblk, occ_rk), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(1), s>>>(UpdateArgs(), a);
+  }
+  static void half(const HalfArgs& a, cudaStream_t s) {
+    if (a.nlist <= 0) return;
+    const long n = (long)a.nlist * Order<N>::NF;
+    k_half<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
+  }
+  static void image_update(const ImageArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    k_image_update<real, N><<<persistent_grid(a.nblk, occ_img), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(2), s>>>(a);
+  }
+  static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
+  static void record(const PointArgs& a, cudaStream_t s) {
+    if (a.nr <= 0) return;
+    k_record<real, N><<<(a.nr + 127) / 128, 128, 0, s>>>(a);
+  }
+  static void inject(const PointArgs& a, cudaStream_t s) {
+    if (a.ng <= 0) return;
+    const long n = (long)a.ng * Order<N>::Np;
+    k_inject<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
+  }
+  static void capture(const CaptureArgs& a, cudaStream_t s) {
+    if (a.nfaces <= 0) return;
+    const long n = (long)a.nfaces * Order<N>::Nfp;
+    k_capture<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
+  }
+};
+template <typename real> int Launch<real>::occ_rhs = 1;
+template <typename real> int Launch<real>::occ_upd = 1;
+template <typename real> int Launch<real>::occ_rk = 1;
+template <typename real> int Launch<real>::occ_img = 1;
+
+template <typename real> KernelTable make_table(int precision) {
+  KernelTable t;
+  t.N = N; t.precision = precision; t.Np = Order<N>::Np; t.Nfp = Order<N>::Nfp;
+  t.rhs = Launch<real>::rhs; t.update = Launch<real>::update; t.rk = Launch<real>::rk;
+  t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
+  t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
+  t.capture = Launch<real>::capture; t.init = Launch<real>::init;
+  return t;
+}
+
+}  // namespace
+
+#define DG_CAT2(a, b) a##b
+#define DG_CAT(a, b) DG_CAT2(a, b)
+const KernelTable* DG_CAT(dg_kernel_table_order, DG_ORDER)(int precision) {
+  static const KernelTable t32 = make_table<float>(32);
+  static const KernelTable t64 = make_table<double>(64);
+  return precision == 32 ? &t32 : &t64;
+}
+
+}  // namespace dgrtm
