@@ -168,6 +168,14 @@ int rtm_get_fields(dg_ctx* ctx, int which, double* q /* [K][4][Np] */);
 /* ---- measurement ------------------------------------------------------------------------------
  * Counts of kernels launched by this ctx since creation (bench.py's gpu_launches). */
 int dg_get_launch_count(const dg_ctx* ctx, int64_t* n);
+/* Per-kernel timing.  dg_set_profiling(ctx, 1): every following kernel launch of this ctx is bracketed by
+ * a CUDA event pair on the bound stream (adds ~2 us per launch; off by default).  dg_get_kernel_times
+ * synchronises, sums the elapsed milliseconds and the launch counts per kernel class since the last
+ * call into ms[DG_KC_COUNT], count[DG_KC_COUNT] and forgets the events. */
+enum { DG_KC_RHS = 0, DG_KC_UPDATE, DG_KC_HALF, DG_KC_IMAGE_UPDATE, DG_KC_SOURCE, DG_KC_RECORD,
+       DG_KC_INJECT, DG_KC_CAPTURE, DG_KC_RK, DG_KC_COUNT };
+int dg_set_profiling(dg_ctx* ctx, int on);
+int dg_get_kernel_times(dg_ctx* ctx, double* ms, int64_t* count);
 /* Enqueue `reps` launches of one kernel over the whole mesh on the bound stream (state is disturbed:
  * for kernel timing only).  which: 0 volume, 1 surface, 2 fused volume+surface, 3 update (18),
  * 4 backward update with fused imaging (two wavefields). */

@@ -25,6 +25,7 @@ DG_INTEGRATOR_AB3, DG_INTEGRATOR_LSERK4 = 0, 1
 DG_WAVELET_RICKER = 0
 DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
 DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
+KERNEL_CLASSES = ("rhs", "update", "half", "image_update", "source", "record", "inject", "capture", "rk")
 
 _vp, _i, _i64, _d, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_size_t
 _pd = C.POINTER(C.c_double)
@@ -74,6 +75,8 @@ SIGNATURES = {
     "rtm_get_traces": (_i, [_vp, _i, _i64, _pd]),
     "rtm_get_fields": (_i, [_vp, _i, _pd]),
     "dg_get_launch_count": (_i, [_vp, _pi64]),
+    "dg_set_profiling": (_i, [_vp, _i]),
+    "dg_get_kernel_times": (_i, [_vp, _pd, _pi64]),
     "dg_bench_kernel": (_i, [_vp, _i, _i]),
 }
 for _name, (_res, _args) in SIGNATURES.items():
@@ -323,6 +326,16 @@ class DG:
         n = _i64()
         self._ck(_lib.dg_get_launch_count(self._h, C.byref(n)))
         return n.value
+
+    def dg_set_profiling(self, on):
+        self._ck(_lib.dg_set_profiling(self._h, int(bool(on))))
+
+    def dg_get_kernel_times(self):
+        """{kernel class name: (milliseconds, launches)} since the last call (profiling mode)."""
+        ms = np.zeros(len(KERNEL_CLASSES))
+        cnt = np.zeros(len(KERNEL_CLASSES), dtype=np.int64)
+        self._ck(_lib.dg_get_kernel_times(self._h, _ptr(ms, _pd), _ptr(cnt, _pi64)))
+        return {n: (float(ms[i]), int(cnt[i])) for i, n in enumerate(KERNEL_CLASSES)}
 
     def dg_bench_kernel(self, which, reps):
         self._ck(_lib.dg_bench_kernel(self._h, int(which), int(reps)))

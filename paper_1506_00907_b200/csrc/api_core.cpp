@@ -167,8 +167,7 @@ void refresh_traces(dg_ctx* c, Field& F) {
   u.q = F.q; u.qf = F.qf; u.h0 = F.hist[0]; u.h1 = F.hist[1]; u.h2 = F.hist[2];
   u.geo = c->geo; u.wperm = c->wperm; u.blk0 = 0; u.nblk = (int)c->model.nblocks;
   u.c0 = u.c1 = u.c2 = 0; u.ops = c->ops;
-  c->kt->update(u, c->stream);
-  c->launches++;
+  DG_LAUNCH(c, KC_UPDATE, c->kt->update(u, c->stream));
 }
 
 }  // namespace dgrtm
@@ -220,6 +219,11 @@ int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, co
 }
 
 void dg_destroy(dg_ctx* ctx) { delete ctx; }
+} // extern C
+dg_ctx::~dg_ctx() {
+  for (dgrtm::ProfEvent& e : prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+}
+extern "C" {
 
 int dg_set_model(dg_ctx* ctx, const double* rho, const double* c, int nlevels, double cfl) {
   DG_TRY(ctx)

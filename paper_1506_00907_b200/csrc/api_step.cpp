@@ -20,7 +20,7 @@ void launch_update(dg_ctx* c, Field& F, int l, double dts) {
   u.blk0 = c->model.lvl_blk0[l]; u.nblk = c->model.lvl_nblk[l];
   u.c0 = dts * co.a[0]; u.c1 = dts * co.a[1]; u.c2 = dts * co.a[2];      // eq (18)
   u.ops = c->ops;
-  if (u.nblk > 0) { c->kt->update(u, c->stream); c->launches++; }
+  if (u.nblk > 0) DG_LAUNCH(c, KC_UPDATE, c->kt->update(u, c->stream));
 }
 
 void launch_half(dg_ctx* c, Field& F, int l, double dts) {
@@ -33,8 +33,7 @@ void launch_half(dg_ctx* c, Field& F, int l, double dts) {
   h.geo = c->geo; h.wperm = c->wperm; h.list = c->d_coarse[l]; h.nlist = n;
   h.c0 = dts * co.b[0]; h.c1 = dts * co.b[1]; h.c2 = dts * co.b[2];      // eq (19)
   h.ops = c->ops;
-  c->kt->half(h, c->stream);
-  c->launches++;
+  DG_LAUNCH(c, KC_HALF, c->kt->half(h, c->stream));
 }
 
 void launch_image_update(dg_ctx* c, Field& S, Field& R, int l, double dts, const RunOpts& o) {
@@ -51,7 +50,7 @@ void launch_image_update(dg_ctx* c, Field& S, Field& R, int l, double dts, const
   for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
   a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
   a.ops = c->ops;
-  if (a.nblk > 0) { c->kt->image_update(a, c->stream); c->launches++; }
+  if (a.nblk > 0) DG_LAUNCH(c, KC_IMAGE, c->kt->image_update(a, c->stream));
 }
 
 PointArgs point_args(dg_ctx* c, const Field& F) {
@@ -76,7 +75,7 @@ void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double
   a.mode = mode; a.dir = dir; a.capture = capture; a.replay = replay;
   a.ext = c->has_ext ? c->ext : nullptr;
   a.ops = c->ops;
-  if (a.nblk > 0) { c->kt->rhs(a, c->stream); c->launches++; }
+  if (a.nblk > 0) DG_LAUNCH(c, KC_RHS, c->kt->rhs(a, c->stream));
 }
 
 void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
@@ -101,8 +100,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       if (off) ab_partial(o.fields[0]->nhist[l], (double)off / stride[l], w);   // reading Q13
       for (int s = 0; s < 3; ++s) p.lw[l][s] = dir * stride[l] * dtl * w[s];
     }
-    c->kt->record(p, c->stream);
-    c->launches++;
+    DG_LAUNCH(c, KC_RECORD, c->kt->record(p, c->stream));
   };
 
   const int64_t nfine = (int64_t)nglobal * nloc;
@@ -123,16 +121,14 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
           PointArgs p = point_args(c, F);
           p.rhs = out; p.src_slot = (int)md.slot_of[c->src_k]; p.src_w = c->d_src_w;
           p.amp_now = ricker(t_start, c->f0, c->tp, c->amp);
-          c->kt->source(p, c->stream);
-          c->launches++;
+          DG_LAUNCH(c, KC_SOURCE, c->kt->source(p, c->stream));
         }
         if (o.inject_field == fi && c->grp_lvl0[l + 1] > c->grp_lvl0[l]) {
           PointArgs p = point_args(c, F);
           p.rhs = out; p.rcv_w = c->d_rcv_w; p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
           p.g0 = c->grp_lvl0[l]; p.ng = c->grp_lvl0[l + 1] - c->grp_lvl0[l];
           p.grp_slot = c->d_grp_slot; p.grp_off = c->d_grp_off; p.grp_rcv = c->d_grp_rcv;
-          c->kt->inject(p, c->stream);
-          c->launches++;
+          DG_LAUNCH(c, KC_INJECT, c->kt->inject(p, c->stream));
         }
         F.nhist[l] = std::min(F.nhist[l] + 1, 3);
       }
@@ -168,8 +164,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       std::memset(&a, 0, sizeof(a));
       a.q = o.fields[0]->q; a.geo = c->geo; a.faces = c->d_stored[l]; a.nfaces = (int)md.stored[l].size();
       a.record = record_ptr(l, jend / stride[l]); a.ops = c->ops;
-      c->kt->capture(a, c->stream);
-      c->launches++;
+      DG_LAUNCH(c, KC_CAPTURE, c->kt->capture(a, c->stream));
     }
   }
   if (o.record && c->nr > 0) sample_receivers(0, jend);
@@ -199,15 +194,13 @@ void run_lserk4(dg_ctx* c, int nsteps) {
         std::memset(&p, 0, sizeof(p));
         p.rhs = r; p.src_slot = (int)md.slot_of[c->src_k]; p.src_w = c->d_src_w;
         p.amp_now = ricker(t + C[st] * dt, c->f0, c->tp, c->amp);
-        c->kt->source(p, c->stream);
-        c->launches++;
+        DG_LAUNCH(c, KC_SOURCE, c->kt->source(p, c->stream));
       }
       RkArgs k;
       std::memset(&k, 0, sizeof(k));
       k.q = F.q; k.qf = F.qf; k.res = c->scratch; k.r = r; k.geo = c->geo; k.wperm = c->wperm;
       k.blk0 = 0; k.nblk = (int)md.nblocks; k.A = A[st]; k.B = B[st]; k.dt = dt; k.ops = c->ops;
-      c->kt->rk(k, c->stream);
-      c->launches++;
+      DG_LAUNCH(c, KC_RK, c->kt->rk(k, c->stream));
     }
   }
 }
@@ -263,6 +256,27 @@ int dg_get_launch_count(const dg_ctx* ctx, int64_t* n) {
   return DG_OK;
 }
 
+int dg_set_profiling(dg_ctx* ctx, int on) {
+  DG_TRY(ctx)
+  ctx->prof = on != 0;
+  DG_CATCH(ctx)
+}
+
+int dg_get_kernel_times(dg_ctx* ctx, double* ms, int64_t* count) {
+  DG_TRY(ctx)
+  if (!ms || !count) throw ApiError(DG_ERR_ARG, "ms / count is NULL");
+  if (ctx->bound) sync_stream(ctx);
+  for (int k = 0; k < KC_COUNT; ++k) { ms[k] = 0; count[k] = 0; }
+  for (ProfEvent& e : ctx->prof_ev) {
+    float t = 0;
+    cuda_check(cudaEventElapsedTime(&t, e.a, e.b), "cudaEventElapsedTime");
+    ms[e.cls] += t; count[e.cls]++;
+    cudaEventDestroy(e.a); cudaEventDestroy(e.b);
+  }
+  ctx->prof_ev.clear();
+  DG_CATCH(ctx)
+}
+
 int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
   DG_TRY(ctx)
   require_bound(ctx);
@@ -280,8 +294,7 @@ int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
         u.q = F.q; u.qf = F.qf; u.h0 = F.hist[0]; u.h1 = F.hist[1]; u.h2 = F.hist[2];
         u.geo = ctx->geo; u.wperm = ctx->wperm; u.blk0 = 0; u.nblk = (int)md.nblocks;
         u.c0 = 1e-30; u.c1 = -1e-30; u.c2 = 1e-30; u.ops = ctx->ops;
-        ctx->kt->update(u, ctx->stream);
-        ctx->launches++;
+        DG_LAUNCH(ctx, KC_UPDATE, ctx->kt->update(u, ctx->stream));
         break;
       }
       case 4: {
@@ -297,8 +310,7 @@ int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
         for (int s = 0; s < 3; ++s) { a.a[s] = co.a[s]; a.abar[s] = co.abar[s]; }
         for (int s = 0; s < 9; ++s) a.C[s] = co.C[s];
         a.e[2] = -1; a.characteristic = 1; a.ops = ctx->ops;
-        ctx->kt->image_update(a, ctx->stream);
-        ctx->launches++;
+        DG_LAUNCH(ctx, KC_IMAGE, ctx->kt->image_update(a, ctx->stream));
         break;
       }
       default: throw ApiError(DG_ERR_ARG, "which must be 0..4");

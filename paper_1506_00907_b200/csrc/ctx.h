@@ -17,6 +17,10 @@ namespace dgrtm {
 
 constexpr int kMaxLevels = 8;
 
+// kernel classes of the launch counter / per-kernel timing (dg_get_kernel_times)
+enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALF, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_COUNT };
+struct ProfEvent { cudaEvent_t a, b; int cls; };
+
 struct ApiError : std::runtime_error {
   int code;
   ApiError(int c, const std::string& m) : std::runtime_error(m), code(c) {}
@@ -138,6 +142,10 @@ struct dg_ctx {
   int final_nsteps = 0;
 
   int64_t launches = 0;
+  // per-kernel timing (dg_set_profiling): one CUDA event pair per launch on the bound stream
+  bool prof = false;
+  std::vector<dgrtm::ProfEvent> prof_ev;
+  ~dg_ctx();
 };
 
 namespace dgrtm {
@@ -176,4 +184,24 @@ void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double
 void carve_workspace(dg_ctx* c, Carver& cv);
 void require_bound(dg_ctx* c);
 
+// counts a launch and, in profiling mode, brackets it with an event pair on the bound stream
+struct LaunchScope {
+  dg_ctx* c; bool on;
+  ProfEvent e;
+  LaunchScope(dg_ctx* ctx, int cls) : c(ctx), on(ctx->prof) {
+    c->launches++;
+    if (on) {
+      e.cls = cls;
+      cuda_check(cudaEventCreate(&e.a), "cudaEventCreate");
+      cuda_check(cudaEventCreate(&e.b), "cudaEventCreate");
+      cudaEventRecord(e.a, c->stream);
+    }
+  }
+  ~LaunchScope() {
+    if (on) { cudaEventRecord(e.b, c->stream); c->prof_ev.push_back(e); }
+  }
+};
+
 }  // namespace dgrtm
+
+#define DG_LAUNCH(ctx_, cls_, call_) do { dgrtm::LaunchScope ls_((ctx_), (cls_)); call_; } while (0)
