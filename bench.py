@@ -61,7 +61,11 @@ def load_peaks():
 # algorithmic traffic per element and launch, in scalars
 # --------------------------------------------------------------------------------------------------
 def algorithmic_scalars(kernel, Np, Nfp):
-    if kernel == "rhs":            # fused volume + surface: q in, neighbour traces in, factors, rhs out
+    if kernel == "step":           # fused rhs + update: q in/out, nbr traces in, 2 rhs in, 1 rhs out, traces out
+        return 20 * Np + 16 * Nfp + 31
+    if kernel == "step_image":     # the same for two wavefields + image read-modify-write
+        return 2 * (20 * Np + 16 * Nfp + 31) + 2 * Np
+    if kernel == "rhs":            # unfused volume + surface: q in, neighbour traces in, factors, rhs out
         return 8 * Np + 8 * Nfp + 31
     if kernel == "update":         # q in/out, three right-hand sides in, exposed traces out
         return 20 * Np + 8 * Nfp
@@ -190,7 +194,7 @@ def profile_kernels(g, T, reps, elems_per_global_step, Np, Nfp, rs, peak, peak_s
     times = g.dg_get_kernel_times()
     g.dg_set_profiling(False)
     ker = {}
-    for name in ("rhs", "update", "image_update"):
+    for name in ("step", "step_image", "rhs", "update", "image_update"):
         ms, n = times[name]
         if not n:
             continue
@@ -351,7 +355,7 @@ def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps):
     rs = cfg["precision"] // 8
     ker = {}
     nb = min(nsteps, 50)
-    for name, fields in (("rhs", 2), ("image_update", 1)):
+    for name, fields in (("step_image", 1),):
         ms, n = times[name]
         if n:
             nbytes = float(nb) * fields * g.K * algorithmic_scalars(name, g.Np, g.Nfp) * rs

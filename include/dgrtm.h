@@ -173,7 +173,7 @@ int dg_get_launch_count(const dg_ctx* ctx, int64_t* n);
  * synchronises, sums the elapsed milliseconds and the launch counts per kernel class since the last
  * call into ms[DG_KC_COUNT], count[DG_KC_COUNT] and forgets the events. */
 enum { DG_KC_RHS = 0, DG_KC_UPDATE, DG_KC_HALF, DG_KC_IMAGE_UPDATE, DG_KC_SOURCE, DG_KC_RECORD,
-       DG_KC_INJECT, DG_KC_CAPTURE, DG_KC_RK, DG_KC_COUNT };
+       DG_KC_INJECT, DG_KC_CAPTURE, DG_KC_RK, DG_KC_STEP, DG_KC_STEP_IMAGE, DG_KC_COUNT };
 int dg_set_profiling(dg_ctx* ctx, int on);
 int dg_get_kernel_times(dg_ctx* ctx, double* ms, int64_t* count);
 /* Enqueue `reps` launches of one kernel over the whole mesh on the bound stream (state is disturbed:

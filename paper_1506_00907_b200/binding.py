@@ -25,7 +25,7 @@ DG_INTEGRATOR_AB3, DG_INTEGRATOR_LSERK4 = 0, 1
 DG_WAVELET_RICKER = 0
 DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
 DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
-KERNEL_CLASSES = ("rhs", "update", "half", "image_update", "source", "record", "inject", "capture", "rk")
+KERNEL_CLASSES = ("rhs", "update", "half", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
 
 _vp, _i, _i64, _d, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_size_t
 _pd = C.POINTER(C.c_double)

@@ -51,6 +51,7 @@ def build(force=False, orders=(1, 2, 3, 4, 5, 6), verbose=False):
         objs.append(obj)
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
             jobs.append([NVCC, "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xptxas", "-v", "-DDG_ORDER=%d" % n,
+                         *os.environ.get("DG_NVCC_FLAGS", "").split(),     # tuning sweeps (-DDG_F3_TO=.. etc.)
                          "-Xcompiler", "-fPIC", "-c", src, "-o", obj])
     missing = [n for n in range(1, 7) if n not in orders]
     stub = os.path.join(OBJ, "kernels_missing.cpp")

@@ -6,6 +6,14 @@
 
 using namespace dgrtm;
 
+namespace dgrtm {
+void upload_point_source(dg_ctx* c) {
+  std::vector<int32_t> idx((size_t)c->model.nslots, -1);
+  if (c->has_src) idx[c->model.slot_of[c->src_k]] = 0;
+  upload_raw(c, c->d_pt_src, idx.data(), idx.size() * 4);
+}
+}  // namespace dgrtm
+
 namespace {
 
 void upload_tables(dg_ctx* c) {
@@ -25,6 +33,20 @@ void upload_tables(dg_ctx* c) {
     for (int n = 0; n < Np; ++n) LT[(size_t)j * Np + n] = re.LIFT[(size_t)n * NF + j];
   upload_real(c, const_cast<void*>(c->ops.D3T), D3T.data(), D3T.size());
   upload_real(c, const_cast<void*>(c->ops.LIFTT), LT.data(), LT.size());
+  {  // step kernel: D3P[m][3][NPAD] = D_{r,s,t}[n][m], LTP[j][NPAD] = LIFT[n][j], zero-padded in n
+    const int npad = c->kt->step_npad;
+    std::vector<double> D3P((size_t)3 * Np * npad, 0.0), LTP((size_t)NF * npad, 0.0);
+    for (int mm = 0; mm < Np; ++mm)
+      for (int n = 0; n < Np; ++n) {
+        D3P[((size_t)mm * 3 + 0) * npad + n] = re.Dr[(size_t)n * Np + mm];
+        D3P[((size_t)mm * 3 + 1) * npad + n] = re.Ds[(size_t)n * Np + mm];
+        D3P[((size_t)mm * 3 + 2) * npad + n] = re.Dt[(size_t)n * Np + mm];
+      }
+    for (int j = 0; j < NF; ++j)
+      for (int n = 0; n < Np; ++n) LTP[(size_t)j * npad + n] = re.LIFT[(size_t)n * NF + j];
+    upload_real(c, c->d_D3P, D3P.data(), D3P.size());
+    upload_real(c, c->d_LTP, LTP.data(), LTP.size());
+  }
   upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);
   upload_raw(c, const_cast<int*>(c->ops.ptab), m.ptab.data(), m.ptab.size() * 4);
 
@@ -84,6 +106,11 @@ void upload_tables(dg_ctx* c) {
     upload_raw(c, c->d_stored[l], sf.data(), sf.size() * 4);
   }
   if (c->has_src) upload_real(c, c->d_src_w, c->src_w.data(), Np);
+  std::vector<unsigned char> flag((size_t)md.nblocks, 0);
+  for (int l = 0; l < md.nlevels; ++l)
+    for (int32_t s : md.coarse_nb[l]) flag[s >> 5] |= 1;
+  upload_raw(c, c->d_blkflag, flag.data(), flag.size());
+  upload_point_source(c);
 }
 
 }  // namespace

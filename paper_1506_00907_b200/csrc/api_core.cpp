@@ -156,7 +156,9 @@ void fields_from_device(dg_ctx* c, double* q, const char* dq) {
 void clear_field(dg_ctx* c, Field& F) {
   cuda_check(cudaMemsetAsync(F.q, 0, field_bytes(c), c->stream), "memset q");
   for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(F.hist[s], 0, field_bytes(c), c->stream), "memset hist");
-  cuda_check(cudaMemsetAsync(F.qf, 0, trace_bytes(c), c->stream), "memset qf");
+  cuda_check(cudaMemsetAsync(F.qfb[0], 0, trace_bytes(c), c->stream), "memset qf");
+  cuda_check(cudaMemsetAsync(F.qfb[1], 0, trace_bytes(c), c->stream), "memset qf");
+  cuda_check(cudaMemsetAsync(F.qfh, 0, trace_bytes(c), c->stream), "memset qf");
   F.reset_history();
 }
 
@@ -168,6 +170,18 @@ void refresh_traces(dg_ctx* c, Field& F) {
   u.geo = c->geo; u.wperm = c->wperm; u.blk0 = 0; u.nblk = (int)c->model.nblocks;
   u.c0 = u.c1 = u.c2 = 0; u.ops = c->ops;
   DG_LAUNCH(c, KC_UPDATE, c->kt->update(u, c->stream));
+  for (int l = 0; l < kMaxLevels; ++l) F.par[l] = 0;
+}
+
+void normalize_traces(dg_ctx* c, Field& F) {
+  const Model& md = c->model;
+  const size_t per_slot = (size_t)4 * c->REC * c->rs;
+  for (int l = 0; l < md.nlevels; ++l) {
+    if (F.par[l] == 0 || md.lvl_nblk[l] == 0) { F.par[l] = 0; continue; }
+    const size_t off = (size_t)md.lvl_blk0[l] * 32 * per_slot, n = (size_t)md.lvl_nblk[l] * 32 * per_slot;
+    cuda_check(cudaMemcpyAsync(F.qfb[0] + off, F.qfb[1] + off, n, cudaMemcpyDeviceToDevice, c->stream), "normalize traces");
+    F.par[l] = 0;
+  }
 }
 
 }  // namespace dgrtm
@@ -281,7 +295,7 @@ int dg_set_source(dg_ctx* ctx, const double x0[3], int wavelet, double f0, doubl
   point_weights(ctx, x0, &ctx->src_k, nullptr, ctx->src_w.data());
   ctx->f0 = f0; ctx->tp = tp; ctx->amp = amp;
   ctx->has_src = true;
-  if (ctx->bound) upload_real(ctx, ctx->d_src_w, ctx->src_w.data(), ctx->Np);
+  if (ctx->bound) { upload_real(ctx, ctx->d_src_w, ctx->src_w.data(), ctx->Np); upload_point_source(ctx); }
   DG_CATCH(ctx)
 }
 
@@ -319,6 +333,16 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
   c->F.q = cv.take(field_bytes(c));
   for (int s = 0; s < 3; ++s) c->F.hist[s] = cv.take(field_bytes(c));
   c->F.qf = cv.take(trace_bytes(c));
+  c->F.qfb[0] = c->F.qf;
+  c->F.qfb[1] = cv.take(trace_bytes(c));
+  c->F.qfh = cv.take(trace_bytes(c));
+  {
+    const int npad = c->kt ? c->kt->step_npad : Np;
+    c->d_D3P = cv.take((size_t)3 * Np * npad * rs);
+    c->d_LTP = cv.take((size_t)NF * npad * rs);
+  }
+  c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks);
+  c->d_pt_src = (int*)cv.take((size_t)md.nslots * 4);
   c->scratch = cv.take(field_bytes(c));
   c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);
   c->d_src_w = cv.take((size_t)Np * rs);
@@ -342,11 +366,13 @@ int dg_workspace_bytes(dg_ctx* ctx, size_t* n) {
     // the carve writes pointers into the ctx: save and restore them so a bound ctx is not disturbed
     OpsDev ops = ctx->ops; char* geo = ctx->geo; int* nbr = ctx->nbr; int* wperm = ctx->wperm; Field F = ctx->F;
     char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w;
+    char* dp = ctx->d_D3P; char* lp = ctx->d_LTP; unsigned char* bf = ctx->d_blkflag; int* ps = ctx->d_pt_src;
     int* dc[kMaxLevels]; int* ds[kMaxLevels];
     for (int l = 0; l < kMaxLevels; ++l) { dc[l] = ctx->d_coarse[l]; ds[l] = ctx->d_stored[l]; }
     carve_workspace(ctx, count);
     ctx->ops = ops; ctx->geo = geo; ctx->nbr = nbr; ctx->wperm = wperm; ctx->F = F;
     ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw;
+    ctx->d_D3P = dp; ctx->d_LTP = lp; ctx->d_blkflag = bf; ctx->d_pt_src = ps;
     for (int l = 0; l < kMaxLevels; ++l) { ctx->d_coarse[l] = dc[l]; ctx->d_stored[l] = ds[l]; }
   }
   *n = count.used;

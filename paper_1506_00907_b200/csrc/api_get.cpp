@@ -106,6 +106,7 @@ int dg_get_traces(dg_ctx* ctx, double* qf) {
   if (!qf) throw ApiError(DG_ERR_ARG, "qf is NULL");
   const int Nfp = ctx->Nfp, REC = ctx->REC;
   std::vector<double> tmp((size_t)ctx->model.nslots * 4 * REC);
+  normalize_traces(ctx, ctx->F);
   download_real(ctx, tmp.data(), ctx->F.qf, tmp.size());
   // device record (slot,f): [p | n.v][Nfp] at the READER's positions mapP[k][f][i]  ->  owner order
   for (int64_t s = 0; s < ctx->model.nslots; ++s) {

@@ -51,21 +51,28 @@ void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
   c->R.q = cv.take(field_bytes(c));
   for (int s = 0; s < 3; ++s) c->R.hist[s] = cv.take(field_bytes(c));
   c->R.qf = cv.take(trace_bytes(c));
+  c->R.qfb[0] = c->R.qf;
+  c->R.qfb[1] = cv.take(trace_bytes(c));
+  c->R.qfh = cv.take(trace_bytes(c));
+  c->d_pt_rcv = (int*)cv.take((size_t)md.nslots * 4);
+  c->d_pt_val = cv.take(nr * Np * rs);
   c->image = cv.take((size_t)md.nblocks * Np * 32 * rs);
   c->qfinal = cv.take(field_bytes(c));
 }
 
 struct HistPtrs {   // everything carve_history writes, for save / restore around a size query
-  char* rec[kMaxLevels]; char* d_data; int* a; int* b; char* cc; char* d; int* e; int* f; int* g; Field R; char* image; char* qfinal;
+  char* rec[kMaxLevels]; char* d_data; int* a; int* b; char* cc; char* d; int* e; int* f; int* g; Field R; char* image; char* qfinal; int* ptr; char* ptv;
   void save(const dg_ctx* c) {
     for (int l = 0; l < kMaxLevels; ++l) rec[l] = c->rec[l];
     d_data = c->d_data; a = c->d_rcv_slot; b = c->d_rcv_level; cc = c->d_rcv_row; d = c->d_rcv_w;
     e = c->d_grp_slot; f = c->d_grp_off; g = c->d_grp_rcv; R = c->R; image = c->image; qfinal = c->qfinal;
+    ptr = c->d_pt_rcv; ptv = c->d_pt_val;
   }
   void restore(dg_ctx* c) const {
     for (int l = 0; l < kMaxLevels; ++l) c->rec[l] = rec[l];
     c->d_data = d_data; c->d_rcv_slot = a; c->d_rcv_level = b; c->d_rcv_row = cc; c->d_rcv_w = d;
     c->d_grp_slot = e; c->d_grp_off = f; c->d_grp_rcv = g; c->R = R; c->image = image; c->qfinal = qfinal;
+    c->d_pt_rcv = ptr; c->d_pt_val = ptv;
   }
 };
 
@@ -157,6 +164,11 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
     upload_raw(ctx, ctx->d_grp_slot, ctx->grp_slot.data(), ctx->grp_slot.size() * 4);
     upload_raw(ctx, ctx->d_grp_off, ctx->grp_off.data(), ctx->grp_off.size() * 4);
     upload_raw(ctx, ctx->d_grp_rcv, ctx->grp_rcv.data(), ctx->grp_rcv.size() * 4);
+  }
+  {
+    std::vector<int32_t> idx((size_t)ctx->model.nslots, -1);
+    for (size_t g = 0; g < ctx->grp_slot.size(); ++g) idx[ctx->grp_slot[g]] = (int32_t)g;
+    upload_raw(ctx, ctx->d_pt_rcv, idx.data(), idx.size() * 4);
   }
   ctx->hist_bound = true;
   clear_field(ctx, ctx->R);

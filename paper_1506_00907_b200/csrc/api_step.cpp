@@ -78,11 +78,17 @@ void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double
   if (a.nblk > 0) DG_LAUNCH(c, KC_RHS, c->kt->rhs(a, c->stream));
 }
 
+// Algorithm 1 on the fused step kernel: per fine step ONE launch advances every level that sits at the
+// step start (right-hand side at t_start, update to t_start + dt_l, traces into the level's other buffer,
+// half-step traces for finer neighbours); readers pick, per neighbour level, the buffer holding the traces
+// at t_start: the level's current buffer if that level is also at t_start, else (a coarser level in
+// mid-step) its half-step buffer (eq (19)).
 void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   const Model& md = c->model;
   const int L = md.nlevels, nloc = c->nlocal, dir = o.direction;
   const double dtl = c->dt_local;
   if (c->has_prescribed && !c->has_ext) throw ApiError(DG_ERR_STATE, "prescribed-exterior faces need dg_set_exterior");
+  if (o.nfields == 2 && !c->hist_bound) throw ApiError(DG_ERR_STATE, "two wavefields need the RTM region");
   int stride[kMaxLevels];
   for (int l = 0; l < L; ++l) stride[l] = 1 << (L - 1 - l);
   const int src_level = c->has_src ? md.level[c->src_k] : -1;
@@ -90,81 +96,102 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   auto record_ptr = [&](int l, int64_t j) -> char* {
     return c->rec[l] + (size_t)j * md.stored[l].size() * c->REC * c->rs;
   };
+  // p(x_r) at fine time m BEFORE the launch of fine step m: a level at its step start holds q(t); a level
+  // in mid-step already holds q at the END of its step: p(t) = q_end - dt_l sum_s (a_s - I_s(theta)) r_s
+  // with the interpolant (22) (reading Q13)
   auto sample_receivers = [&](int64_t m, int64_t jabs) {
     PointArgs p = point_args(c, *o.fields[0]);
     p.nr = (int)c->nr; p.rcv_slot = c->d_rcv_slot; p.rcv_row = c->d_rcv_row; p.rcv_level = c->d_rcv_level;
     p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
     for (int l = 0; l < L; ++l) {
       const int off = (int)(m % stride[l]);
+      if (!off) continue;
+      const int order = o.fields[0]->nhist[l];
       double w[3] = {0, 0, 0};
-      if (off) ab_partial(o.fields[0]->nhist[l], (double)off / stride[l], w);   // reading Q13
-      for (int s = 0; s < 3; ++s) p.lw[l][s] = dir * stride[l] * dtl * w[s];
+      ab_partial(order, (double)off / stride[l], w);
+      const AbCoef& co = ab_coef(order);
+      for (int s = 0; s < 3; ++s) p.lw[l][s] = -dir * stride[l] * dtl * (co.a[s] - w[s]);
     }
     DG_LAUNCH(c, KC_RECORD, c->kt->record(p, c->stream));
   };
+
+  StepArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.nfields = o.nfields; a.nlevels = L;
+  a.geo = c->geo; a.nbr = c->nbr; a.wperm = c->wperm; a.blkflag = c->d_blkflag;
+  a.ext = c->has_ext ? c->ext : nullptr;
+  a.dir = (double)dir;
+  a.ops = c->ops; a.ops.D3T = c->d_D3P; a.ops.LIFTT = c->d_LTP;
+  a.image = c->image; a.img_scratch = c->scratch; a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
+  for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
+  for (int fi = 0; fi < o.nfields; ++fi) {
+    a.q[fi] = o.fields[fi]->q;
+    if (o.source_on[fi]) { a.pt_index[fi] = c->d_pt_src; a.pt_val[fi] = c->d_src_w; }
+    if (o.inject_field == fi && !c->grp_slot.empty()) { a.pt_index[fi] = c->d_pt_rcv; a.pt_val[fi] = c->d_pt_val; a.pt_scale[fi] = 1.0; }
+  }
+  for (int l = 0; l < L; ++l) a.lv[l].blk_end = md.lvl_blk0[l] + md.lvl_nblk[l];
 
   const int64_t nfine = (int64_t)nglobal * nloc;
   for (int64_t m = 0; m < nfine; ++m) {
     const int64_t jabs = o.first_fine + dir * m;
     const double t_start = o.t0 + dir * (double)m * dtl;
-    // ---- right-hand sides of every level whose unknowns sit at t_start
+    if (o.record && c->nr > 0) sample_receivers(m, jabs);
+    if (o.inject_field >= 0 && !c->grp_slot.empty()) {     // injection amounts of this fine step (eq (15))
+      PointArgs p = point_args(c, *o.fields[o.inject_field]);
+      p.rcv_w = c->d_rcv_w; p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
+      p.g0 = 0; p.ng = (int)c->grp_slot.size();
+      p.grp_slot = c->d_grp_slot; p.grp_off = c->d_grp_off; p.grp_rcv = c->d_grp_rcv; p.pt_out = c->d_pt_val;
+      DG_LAUNCH(c, KC_INJECT, c->kt->inject(p, c->stream));
+    }
+    int lmin = L - 1;
+    while (lmin > 0 && m % stride[lmin - 1] == 0) --lmin;   // strides are powers of two
     for (int l = 0; l < L; ++l) {
-      if (m % stride[l] != 0 || md.lvl_nblk[l] == 0) continue;
+      StepLevel& S = a.lv[l];
+      const bool active = l >= lmin;
+      S.active = active;
       for (int fi = 0; fi < o.nfields; ++fi) {
         Field& F = *o.fields[fi];
+        // traces at t_start: the current buffer of a level that is at t_start, the half-step buffer otherwise
+        S.qf_read[fi] = active ? F.qfb[F.par[l]] : F.qfh;
+        if (!active) continue;
         F.cur[l] = (F.cur[l] + 1) % 3;
-        char* out = F.hist[F.cur[l]];
-        char* cap = (fi == 0 && o.capture && !md.stored[l].empty()) ? record_ptr(l, jabs / stride[l]) : nullptr;
-        const char* rep = (fi == 0 && o.replay && !md.stored[l].empty()) ? record_ptr(l, jabs / stride[l]) : nullptr;
-        launch_rhs(c, F, out, l, l + 1, RHS_VOL | RHS_SURF, (double)dir, cap, rep);
-        if (o.source_on[fi] && src_level == l) {                       // eq (15), reading Q5
-          PointArgs p = point_args(c, F);
-          p.rhs = out; p.src_slot = (int)md.slot_of[c->src_k]; p.src_w = c->d_src_w;
-          p.amp_now = ricker(t_start, c->f0, c->tp, c->amp);
-          DG_LAUNCH(c, KC_SOURCE, c->kt->source(p, c->stream));
-        }
-        if (o.inject_field == fi && c->grp_lvl0[l + 1] > c->grp_lvl0[l]) {
-          PointArgs p = point_args(c, F);
-          p.rhs = out; p.rcv_w = c->d_rcv_w; p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
-          p.g0 = c->grp_lvl0[l]; p.ng = c->grp_lvl0[l + 1] - c->grp_lvl0[l];
-          p.grp_slot = c->d_grp_slot; p.grp_off = c->d_grp_off; p.grp_rcv = c->d_grp_rcv;
-          DG_LAUNCH(c, KC_INJECT, c->kt->inject(p, c->stream));
-        }
         F.nhist[l] = std::min(F.nhist[l] + 1, 3);
+        S.r0[fi] = F.hist[F.cur[l]]; S.r1[fi] = F.h(l, 1); S.r2[fi] = F.h(l, 2);
+        S.qf_write[fi] = F.qfb[F.par[l] ^ 1];
+        S.qf_half[fi] = (l + 1 < L && !md.coarse_nb[l].empty()) ? F.qfh : nullptr;
       }
-    }
-    if (o.record && c->nr > 0) sample_receivers(m, jabs);
-    // ---- updates (18) of the levels that land on t_new, finest first
-    int coarsest_updated = L;
-    for (int l = L - 1; l >= 0; --l) {
-      if ((m + 1) % stride[l] != 0) continue;
-      coarsest_updated = l;
-      if (md.lvl_nblk[l] == 0) continue;
+      if (!active) continue;
+      const AbCoef& co = ab_coef(o.fields[0]->nhist[l]);
       const double dts = dir * (double)stride[l] * dtl;
-      const int64_t jend = jabs + dir * 1;     // fine index after this fine step
-      const bool img = o.image && std::min(jabs, jend) >= o.image_min_fine;
-      if (img) {
-        launch_image_update(c, *o.fields[0], *o.fields[1], l, dts, o);
-      } else {
-        for (int fi = 0; fi < o.nfields; ++fi) launch_update(c, *o.fields[fi], l, dts);
-      }
+      S.dts = dts;
+      for (int s = 0; s < 3; ++s) { S.c[s] = dts * co.a[s]; S.d[s] = dts * (co.b[s] - co.a[s]); S.abar[s] = co.abar[s]; }
+      for (int s = 0; s < 9; ++s) S.C[s] = co.C[s];
+      const bool stored = !md.stored[l].empty();
+      S.capture = (o.capture && stored) ? record_ptr(l, jabs / stride[l]) : nullptr;
+      S.replay = (o.replay && stored) ? record_ptr(l, jabs / stride[l]) : nullptr;
+      const int64_t jlast = jabs + dir * (stride[l] - 1);   // start of the fine step on which this update lands
+      S.image_on = o.image && std::min(jlast, jlast + dir) >= o.image_min_fine;
     }
-    // ---- coarse neighbours that were not updated: half-step traces (19)
-    const int lc = coarsest_updated - 1;
-    if (lc >= 0 && lc < L) {
-      const double dts = dir * (double)stride[lc] * dtl;
-      for (int fi = 0; fi < o.nfields; ++fi) launch_half(c, *o.fields[fi], lc, dts);
+    for (int fi = 0; fi < o.nfields; ++fi)
+      if (o.source_on[fi]) a.pt_scale[fi] = (src_level >= lmin) ? ricker(t_start, c->f0, c->tp, c->amp) : 0.0;
+    a.blk0 = md.lvl_blk0[lmin];
+    a.nblk = (int)md.nblocks - a.blk0;
+    if (a.nblk > 0) {
+      if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, c->kt->step2(a, c->stream));
+      else DG_LAUNCH(c, KC_STEP, c->kt->step(a, c->stream));
     }
+    for (int l = lmin; l < L; ++l)
+      for (int fi = 0; fi < o.nfields; ++fi) o.fields[fi]->par[l] ^= 1;
   }
   const int64_t jend = o.first_fine + dir * nfine;
   if (o.capture) {
     for (int l = 0; l < L; ++l) {
       if (md.stored[l].empty()) continue;
-      CaptureArgs a;
-      std::memset(&a, 0, sizeof(a));
-      a.q = o.fields[0]->q; a.geo = c->geo; a.faces = c->d_stored[l]; a.nfaces = (int)md.stored[l].size();
-      a.record = record_ptr(l, jend / stride[l]); a.ops = c->ops;
-      DG_LAUNCH(c, KC_CAPTURE, c->kt->capture(a, c->stream));
+      CaptureArgs ca;
+      std::memset(&ca, 0, sizeof(ca));
+      ca.q = o.fields[0]->q; ca.geo = c->geo; ca.faces = c->d_stored[l]; ca.nfaces = (int)md.stored[l].size();
+      ca.record = record_ptr(l, jend / stride[l]); ca.ops = c->ops;
+      DG_LAUNCH(c, KC_CAPTURE, c->kt->capture(ca, c->stream));
     }
   }
   if (o.record && c->nr > 0) sample_receivers(0, jend);
@@ -183,6 +210,7 @@ void run_lserk4(dg_ctx* c, int nsteps) {
   if (md.nlevels != 1) throw ApiError(DG_ERR_UNSUPPORTED, "LSERK4 is single-rate only");
   if (c->has_prescribed && !c->has_ext) throw ApiError(DG_ERR_STATE, "prescribed-exterior faces need dg_set_exterior");
   Field& F = c->F;
+  normalize_traces(c, F);
   const double dt = c->dt_local;
   for (int n = 0; n < nsteps; ++n) {
     const double t = c->t0 + (double)(c->fine + n) * dt;
@@ -244,6 +272,7 @@ int dg_get_rhs(dg_ctx* ctx, int which, int direction, double* r) {
   }
   // the scratch array doubles as the LSERK4 residual, which is dead between steps (A_1 = 0)
   cuda_check(cudaMemsetAsync(ctx->scratch, 0, field_bytes(ctx), ctx->stream), "memset scratch");
+  normalize_traces(ctx, ctx->F);
   launch_rhs(ctx, ctx->F, ctx->scratch, 0, ctx->model.nlevels, mode, (double)direction, nullptr, nullptr);
   cuda_check(cudaGetLastError(), "kernel launch");
   fields_from_device(ctx, r, ctx->scratch);
@@ -283,6 +312,7 @@ int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
   if (reps < 0) throw ApiError(DG_ERR_ARG, "reps must be >= 0");
   const Model& md = ctx->model;
   Field& F = ctx->F;
+  normalize_traces(ctx, F);
   for (int i = 0; i < reps; ++i) {
     switch (which) {
       case 0: launch_rhs(ctx, F, F.hist[0], 0, md.nlevels, RHS_VOL, 1.0, nullptr, nullptr); break;

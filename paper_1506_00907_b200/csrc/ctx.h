@@ -18,7 +18,7 @@ namespace dgrtm {
 constexpr int kMaxLevels = 8;
 
 // kernel classes of the launch counter / per-kernel timing (dg_get_kernel_times)
-enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALF, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_COUNT };
+enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALF, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_STEP, KC_STEP_IMAGE, KC_COUNT };
 struct ProfEvent { cudaEvent_t a, b; int cls; };
 
 struct ApiError : std::runtime_error {
@@ -35,11 +35,15 @@ inline void cuda_check(cudaError_t e, const char* what) {
 struct Field {
   char* q = nullptr;
   char* hist[3] = {nullptr, nullptr, nullptr};
-  char* qf = nullptr;
+  char* qf = nullptr;      // = qfb[0]: the array the unfused kernels (k_rhs, k_update, k_half) use
+  // fused step kernel: traces double-buffered per level + half-step traces of coarse neighbours
+  char* qfb[2] = {nullptr, nullptr};
+  char* qfh = nullptr;
+  int par[kMaxLevels];     // per level: which of qfb[] holds the level's current traces
   int cur[kMaxLevels];     // per level: which of hist[] holds the newest right-hand side
   int nhist[kMaxLevels];   // per level: number of valid history entries (start-up order, reading Q7)
   void reset_history() {
-    for (int l = 0; l < kMaxLevels; ++l) { cur[l] = 0; nhist[l] = 0; }
+    for (int l = 0; l < kMaxLevels; ++l) { cur[l] = 0; nhist[l] = 0; par[l] = 0; }
   }
   const char* h(int l, int s) const { return hist[(cur[l] + 3 - s) % 3]; }   // s = 0 newest
 };
@@ -116,6 +120,10 @@ struct dg_ctx {
   char* ext = nullptr;                      // prescribed exterior states [nbnd][Nfp][2]
   bool has_ext = false;
   char* d_src_w = nullptr;
+  char* d_D3P = nullptr;                    // step kernel's padded operator tables [m][3][NPAD], [j][NPAD]
+  char* d_LTP = nullptr;
+  unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour
+  int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
   int* d_coarse[dgrtm::kMaxLevels];         // per level: slots with a finer face neighbour
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
@@ -135,6 +143,8 @@ struct dg_ctx {
   int* d_grp_slot = nullptr;
   int* d_grp_off = nullptr;
   int* d_grp_rcv = nullptr;
+  int* d_pt_rcv = nullptr;                  // per slot: receiver group of the element or -1
+  char* d_pt_val = nullptr;                 // [ngroups][Np] injection amounts of the current fine step
   dgrtm::Field R;                           // receiver wavefield of the backward phase
   char* image = nullptr;
   char* qfinal = nullptr;
@@ -161,6 +171,8 @@ void sync_stream(dg_ctx* c);
 void fields_to_device(dg_ctx* c, char* dq, const double* q);
 void fields_from_device(dg_ctx* c, double* q, const char* dq);
 void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
+void normalize_traces(dg_ctx* c, Field& F);
+void upload_point_source(dg_ctx* c);        // per-slot point-term index of the forward field // current traces of every level -> qfb[0] (= qf)
 void clear_field(dg_ctx* c, Field& F);
 
 struct RunOpts {

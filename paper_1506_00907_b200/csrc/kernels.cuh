@@ -506,7 +506,8 @@ __global__ void k_inject(PointArgs a) {
     const int r = a.grp_rcv[x];
     acc += data[(size_t)r * a.nsamp + a.sample] * w[(size_t)r * Np + n];
   }
-  static_cast<real*>(a.rhs)[(size_t)b * (4 * Np * 32) + (size_t)n * 32 + lane] += acc;
+  if (a.pt_out) static_cast<real*>(a.pt_out)[(size_t)g * Np + n] = acc;       // fused step kernel adds it
+  else static_cast<real*>(a.rhs)[(size_t)b * (4 * Np * 32) + (size_t)n * 32 + lane] += acc;
 }
 
 }  // namespace dgrtm

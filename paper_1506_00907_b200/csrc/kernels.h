@@ -92,10 +92,50 @@ struct PointArgs {         // source term / receiver sampling / receiver injecti
   double lw[8][3];         // per level: signed-step-scaled partial AB weights (reading Q13)
   // injection groups
   int g0, ng; const int* grp_slot; const int* grp_off; const int* grp_rcv;
+  void* pt_out;            // if set: injection amounts go to pt_out[group][Np] instead of into rhs
 };
 
 struct CaptureArgs {       // own traces of a list of (slot*4+f) faces -> record
   const void* q; const void* geo; const int* faces; int nfaces; void* record; OpsDev ops;
+};
+
+// ---- fused step kernel (step_kernel.cuh) ---------------------------------------------------------
+// One launch advances every level that sits at the start of the fine step.  Per level (contiguous block
+// range): where its right-hand sides rotate, where its traces are read / written, its AB weights.
+struct StepLevel {
+  int blk_end;               // first block past this level
+  int active;                // evaluated and updated by this launch
+  int image_on;              // this step contributes to the image (two-field launches)
+  int pad_;
+  void* r0[2];               // per field: newest right-hand side (written)
+  const void* r1[2];         // per field: the two older ones (read)
+  const void* r2[2];
+  const void* qf_read[2];    // per field: traces of this level's elements AT THE STEP START, as seen by readers
+  void* qf_write[2];         // per field: traces at the end of this level's step
+  void* qf_half[2];          // per field: half-step traces (19) for finer neighbours (null: none needed)
+  void* capture;             // field 0: boundary-trace record written at this evaluation, or null
+  const void* replay;        // field 0: record read as exterior state of the stored faces, or null
+  double c[3];               // dts * a_s   (eq (18))
+  double d[3];               // dts * (b_s - a_s): half-step value = updated value + sum d_s r_s  (eq (19))
+  double dts;                // signed local step
+  double abar[3], C[9];      // image weights of the AB order in use (eqs (22)-(24), reading Q1)
+};
+
+struct StepArgs {
+  void* q[2];                // nodal values of field 0 (source / forward) and field 1 (receivers)
+  int nfields;
+  int blk0, nblk;            // block range covered by the launch (levels l_min .. L-1)
+  int nlevels;
+  const void* geo; const int* nbr; const int* wperm;
+  const unsigned char* blkflag;   // per block: bit 0 = some element has a finer face neighbour
+  const void* ext;           // prescribed exterior states or null
+  double dir;
+  // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale
+  const int* pt_index[2]; const void* pt_val[2]; double pt_scale[2];
+  void* image; double e[3]; int characteristic;
+  void* img_scratch;         // [block][4Np][32] scratch for the imaging scalars when they do not fit in shared memory
+  OpsDev ops;                // D3T / LIFTT here are the PADDED tables: D3P [m][3][NPAD], LTP [j][NPAD]
+  StepLevel lv[8];
 };
 
 struct KernelTable {
@@ -109,6 +149,9 @@ struct KernelTable {
   void (*record)(const PointArgs&, cudaStream_t);
   void (*inject)(const PointArgs&, cudaStream_t);
   void (*capture)(const CaptureArgs&, cudaStream_t);
+  void (*step)(const StepArgs&, cudaStream_t);        // one wavefield
+  void (*step2)(const StepArgs&, cudaStream_t);       // two wavefields + imaging
+  int step_npad;                                       // padded output count of the step kernel's tables
   int (*init)();           // sets shared-memory attributes; returns cudaError
 };
 

@@ -1,5 +1,5 @@
 // One translation unit per order: compiled six times with -DDG_ORDER=1..6 (float and double each).
-#include "kernels.cuh"
+#include "step_kernel.cuh"
 
 #ifndef DG_ORDER
 #error "compile with -DDG_ORDER=<1..6>"
@@ -38,6 +38,12 @@ template <typename real> struct Launch {
     e = cudaFuncSetAttribute(k_image_update<real, N>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)UpdSmem<N>::template bytes<real>(2));
     if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_step<real, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)StepSmem<real, N, false>::bytes);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaFuncSetAttribute(k_step<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)StepSmem<real, N, true>::bytes);
+    if (e != cudaSuccess) return (int)e;
     const int th = 32 * Tiling<N>::T;
     occ_rhs = blocks_per_sm(k_rhs<real, N>, th, RhsSmem<real, N>::bytes);
     occ_upd = blocks_per_sm(k_update<real, N, 0>, th, UpdSmem<N>::template bytes<real>(1));
@@ -65,6 +71,16 @@ template <typename real> struct Launch {
   static void image_update(const ImageArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     k_image_update<real, N><<<persistent_grid(a.nblk, occ_img), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(2), s>>>(a);
+  }
+  static void step(const StepArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    using SM = StepSmem<real, N, false>;
+    k_step<real, N, false><<<a.nblk < kSMs ? a.nblk : kSMs, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
+  }
+  static void step2(const StepArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    using SM = StepSmem<real, N, true>;
+    k_step<real, N, true><<<a.nblk < kSMs ? a.nblk : kSMs, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
   }
   static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
   static void record(const PointArgs& a, cudaStream_t s) {
@@ -94,6 +110,7 @@ template <typename real> KernelTable make_table(int precision) {
   t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
   t.capture = Launch<real>::capture; t.init = Launch<real>::init;
+  t.step = Launch<real>::step; t.step2 = Launch<real>::step2; t.step_npad = StepSmem<real, N, false>::NPAD;
   return t;
 }
 
