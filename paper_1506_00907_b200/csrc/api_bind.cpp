@@ -46,6 +46,22 @@ void upload_tables(dg_ctx* c) {
       for (int n = 0; n < Np; ++n) LTP[(size_t)j * npad + n] = re.LIFT[(size_t)n * NF + j];
     upload_real(c, c->d_D3P, D3P.data(), D3P.size());
     upload_real(c, c->d_LTP, LTP.data(), LTP.size());
+    if (c->kt->pipe) {   // tile-packed: D3Q[w][m][RL] = (Dr, Ds, Dt)[n0 + nn][m], LTQ[w][j][LL] = LIFT[n0 + nn][j]
+      const int TO = c->kt->pipe_TO, NT = c->kt->pipe_NT, RL = c->kt->pipe_RL, LL = c->kt->pipe_LL;
+      std::vector<double> D3Q((size_t)NT * Np * RL, 0.0), LTQ((size_t)NT * NF * LL, 0.0);
+      for (int w = 0; w < NT; ++w)
+        for (int nn = 0; nn < TO; ++nn) {
+          const int n = w * TO + nn;
+          if (n >= Np) continue;
+          for (int mm = 0; mm < Np; ++mm) {
+            double* row = &D3Q[((size_t)w * Np + mm) * RL];
+            row[nn] = re.Dr[(size_t)n * Np + mm]; row[TO + nn] = re.Ds[(size_t)n * Np + mm]; row[2 * TO + nn] = re.Dt[(size_t)n * Np + mm];
+          }
+          for (int j = 0; j < NF; ++j) LTQ[((size_t)w * NF + j) * LL + nn] = re.LIFT[(size_t)n * NF + j];
+        }
+      upload_real(c, c->d_D3Q, D3Q.data(), D3Q.size());
+      upload_real(c, c->d_LTQ, LTQ.data(), LTQ.size());
+    }
   }
   upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);
   upload_raw(c, const_cast<int*>(c->ops.ptab), m.ptab.data(), m.ptab.size() * 4);

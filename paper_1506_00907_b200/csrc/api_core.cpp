@@ -1,6 +1,7 @@
 // C ABI of libdgrtm, part 1: context, setup, device workspace (include/dgrtm.h).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <mutex>
 
 #include "ctx.h"
@@ -223,6 +224,7 @@ int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, co
     c->kt = get_kernel_table(N, precision);
     for (int l = 0; l < kMaxLevels; ++l) { c->d_coarse[l] = nullptr; c->d_stored[l] = nullptr; c->rec[l] = nullptr; }
     c->F.reset_history(); c->R.reset_history();
+    if (const char* k = std::getenv("DGRTM_KERNEL")) c->use_pipe = std::string(k) != "step";
   } catch (const std::exception& e) {
     g_create_error = e.what();
     delete c;
@@ -340,6 +342,9 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
     const int npad = c->kt ? c->kt->step_npad : Np;
     c->d_D3P = cv.take((size_t)3 * Np * npad * rs);
     c->d_LTP = cv.take((size_t)NF * npad * rs);
+    const int nt = c->kt ? c->kt->pipe_NT : 0;
+    c->d_D3Q = cv.take((size_t)std::max(1, nt * Np * (c->kt ? c->kt->pipe_RL : 0)) * rs);
+    c->d_LTQ = cv.take((size_t)std::max(1, nt * NF * (c->kt ? c->kt->pipe_LL : 0)) * rs);
   }
   c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks);
   c->d_pt_src = (int*)cv.take((size_t)md.nslots * 4);
@@ -366,13 +371,13 @@ int dg_workspace_bytes(dg_ctx* ctx, size_t* n) {
     // the carve writes pointers into the ctx: save and restore them so a bound ctx is not disturbed
     OpsDev ops = ctx->ops; char* geo = ctx->geo; int* nbr = ctx->nbr; int* wperm = ctx->wperm; Field F = ctx->F;
     char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w;
-    char* dp = ctx->d_D3P; char* lp = ctx->d_LTP; unsigned char* bf = ctx->d_blkflag; int* ps = ctx->d_pt_src;
+    char* dp = ctx->d_D3P; char* lp = ctx->d_LTP; char* dq = ctx->d_D3Q; char* lq = ctx->d_LTQ; unsigned char* bf = ctx->d_blkflag; int* ps = ctx->d_pt_src;
     int* dc[kMaxLevels]; int* ds[kMaxLevels];
     for (int l = 0; l < kMaxLevels; ++l) { dc[l] = ctx->d_coarse[l]; ds[l] = ctx->d_stored[l]; }
     carve_workspace(ctx, count);
     ctx->ops = ops; ctx->geo = geo; ctx->nbr = nbr; ctx->wperm = wperm; ctx->F = F;
     ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw;
-    ctx->d_D3P = dp; ctx->d_LTP = lp; ctx->d_blkflag = bf; ctx->d_pt_src = ps;
+    ctx->d_D3P = dp; ctx->d_LTP = lp; ctx->d_D3Q = dq; ctx->d_LTQ = lq; ctx->d_blkflag = bf; ctx->d_pt_src = ps;
     for (int l = 0; l < kMaxLevels; ++l) { ctx->d_coarse[l] = dc[l]; ctx->d_stored[l] = ds[l]; }
   }
   *n = count.used;

@@ -122,6 +122,8 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.ext = c->has_ext ? c->ext : nullptr;
   a.dir = (double)dir;
   a.ops = c->ops; a.ops.D3T = c->d_D3P; a.ops.LIFTT = c->d_LTP;
+  a.ops2_D3Q = c->d_D3Q; a.ops2_LTQ = c->d_LTQ;
+  const bool pipe = c->use_pipe && c->kt->pipe != nullptr;
   a.image = c->image; a.img_scratch = c->scratch; a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
   for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
   for (int fi = 0; fi < o.nfields; ++fi) {
@@ -177,8 +179,8 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     a.blk0 = md.lvl_blk0[lmin];
     a.nblk = (int)md.nblocks - a.blk0;
     if (a.nblk > 0) {
-      if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, c->kt->step2(a, c->stream));
-      else DG_LAUNCH(c, KC_STEP, c->kt->step(a, c->stream));
+      if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, pipe ? c->kt->pipe2(a, c->stream) : c->kt->step2(a, c->stream));
+      else DG_LAUNCH(c, KC_STEP, pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream));
     }
     for (int l = lmin; l < L; ++l)
       for (int fi = 0; fi < o.nfields; ++fi) o.fields[fi]->par[l] ^= 1;

@@ -122,6 +122,9 @@ struct dg_ctx {
   char* d_src_w = nullptr;
   char* d_D3P = nullptr;                    // step kernel's padded operator tables [m][3][NPAD], [j][NPAD]
   char* d_LTP = nullptr;
+  char* d_D3Q = nullptr;                    // pipelined kernel's tile-packed tables
+  char* d_LTQ = nullptr;
+  bool use_pipe = true;                     // DGRTM_KERNEL=step selects the non-pipelined fused kernel
   unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
   int* d_coarse[dgrtm::kMaxLevels];         // per level: slots with a finer face neighbour

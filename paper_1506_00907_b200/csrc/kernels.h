@@ -135,6 +135,8 @@ struct StepArgs {
   void* image; double e[3]; int characteristic;
   void* img_scratch;         // [block][4Np][32] scratch for the imaging scalars when they do not fit in shared memory
   OpsDev ops;                // D3T / LIFTT here are the PADDED tables: D3P [m][3][NPAD], LTP [j][NPAD]
+  const void* ops2_D3Q;      // pipelined kernel: tile-packed tables D3Q [tile][m][RL], LTQ [tile][j][LL]
+  const void* ops2_LTQ;
   StepLevel lv[8];
 };
 
@@ -152,6 +154,10 @@ struct KernelTable {
   void (*step)(const StepArgs&, cudaStream_t);        // one wavefield
   void (*step2)(const StepArgs&, cudaStream_t);       // two wavefields + imaging
   int step_npad;                                       // padded output count of the step kernel's tables
+  // software-pipelined variant (pipe_kernel.cuh); pipe == nullptr if not instantiated for this (N, precision)
+  void (*pipe)(const StepArgs&, cudaStream_t);
+  void (*pipe2)(const StepArgs&, cudaStream_t);
+  int pipe_TO, pipe_NT, pipe_RL, pipe_LL;
   int (*init)();           // sets shared-memory attributes; returns cudaError
 };
 

@@ -1,5 +1,5 @@
 // One translation unit per order: compiled six times with -DDG_ORDER=1..6 (float and double each).
-#include "step_kernel.cuh"
+#include "pipe_kernel.cuh"
 
 #ifndef DG_ORDER
 #error "compile with -DDG_ORDER=<1..6>"
@@ -44,6 +44,12 @@ template <typename real> struct Launch {
     e = cudaFuncSetAttribute(k_step<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)StepSmem<real, N, true>::bytes);
     if (e != cudaSuccess) return (int)e;
+    if constexpr (PipeCfg<real, N>::enabled) {
+      e = cudaFuncSetAttribute(k_pipe<real, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PipeSmem<real, N>::bytes);
+      if (e != cudaSuccess) return (int)e;
+      e = cudaFuncSetAttribute(k_pipe<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PipeSmem<real, N>::bytes);
+      if (e != cudaSuccess) return (int)e;
+    }
     const int th = 32 * Tiling<N>::T;
     occ_rhs = blocks_per_sm(k_rhs<real, N>, th, RhsSmem<real, N>::bytes);
     occ_upd = blocks_per_sm(k_update<real, N, 0>, th, UpdSmem<N>::template bytes<real>(1));
@@ -82,6 +88,16 @@ template <typename real> struct Launch {
     using SM = StepSmem<real, N, true>;
     k_step<real, N, true><<<a.nblk < kSMs ? a.nblk : kSMs, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
   }
+  static void pipe(const StepArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    using C = PipeCfg<real, N>;
+    k_pipe<real, N, false><<<a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s>>>(a);
+  }
+  static void pipe2(const StepArgs& a, cudaStream_t s) {
+    if (a.nblk <= 0) return;
+    using C = PipeCfg<real, N>;
+    k_pipe<real, N, true><<<a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s>>>(a);
+  }
   static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
   static void record(const PointArgs& a, cudaStream_t s) {
     if (a.nr <= 0) return;
@@ -110,6 +126,12 @@ template <typename real> KernelTable make_table(int precision) {
   t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
   t.capture = Launch<real>::capture; t.init = Launch<real>::init;
+  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0;
+  if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
+    t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
+    t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;
+    t.pipe_RL = PipeSmem<real, N>::RL; t.pipe_LL = PipeSmem<real, N>::LL;
+  }
   t.step = Launch<real>::step; t.step2 = Launch<real>::step2; t.step_npad = StepSmem<real, N, false>::NPAD;
   return t;
 }

@@ -1,0 +1,435 @@
+// k_pipe: the fused step of step_kernel.cuh as a software pipeline.  Same arithmetic, same StepArgs;
+// what changes is how operands reach the SM:
+//   * every contiguous input of a work item (one 32-element block of one wavefield) - q, the two older
+//     right-hand sides, the geometric factors - arrives by cp.async.bulk (TMA, 1-D) in a two-stage shared
+//     memory ring, issued one item ahead and completed on an mbarrier;
+//   * the neighbours' trace records (an indirect gather, one record per lane and face) arrive by per-lane
+//     cp.async (LDGSTS) one item ahead, issued and consumed by the same lane;
+//   * the consumer warps therefore never wait on a global load: they read shared memory, issue FMAs and
+//     fire-and-forget stores (new right-hand side, new q, new traces).
+// Operator tables are packed per output tile: D3Q[tile][m][RL] = Dr[n0..][m], Ds[..][m], Dt[..][m] (RL =
+// 3 TO rounded up to the vector width), LTQ[tile][j][LL], so every operator fetch is a full-width LDS.
+#pragma once
+#include "step_kernel.cuh"
+
+namespace dgrtm {
+
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1; };
+#ifndef DG_P3_TO
+#define DG_P3_TO 5
+#define DG_P3_NT 4
+#define DG_P3_G 2
+#endif
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G; };
+
+template <typename real, int N> struct PipeSmem {
+  using O = Order<N>;
+  using C = PipeCfg<real, N>;
+  static constexpr int VW = 16 / (int)sizeof(real);
+  static constexpr int RL = (3 * C::TO + VW - 1) / VW * VW;        // packed derivative row
+  static constexpr int LL = (C::TO + VW - 1) / VW * VW;            // packed lift row
+  static constexpr size_t ops_reals = (size_t)C::NT * O::Np * RL + (size_t)C::NT * O::NF * LL;
+  static constexpr size_t tab_ints = O::NF + 3 * O::Np + UpdSmem<N>::kMaxPerm * O::Nfp;
+  static constexpr size_t ops_bytes = (ops_reals * sizeof(real) + tab_ints * sizeof(int) + 127) / 128 * 128;
+  // one stage: q, r1, r2 [4Np][32] each, factors [DG_NGEO][32], neighbour records [4][32][REC]
+  static constexpr size_t stage_reals = (size_t)(12 * O::Np + DG_NGEO + 4 * O::REC) * 32;
+  static constexpr size_t group_reals = 2 * stage_reals + (size_t)2 * O::NF * 32;      // + penalties / staging
+  static constexpr size_t group_bytes = group_reals * sizeof(real);
+  static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
+  static constexpr bool fits = bytes <= 227 * 1024;
+};
+
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* dst, const void* src) {
+  if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+  else if (BYTES == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+// full-width vector loads of a packed operator row
+template <typename real, int LEN>
+__device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&out)[LEN]) {
+  constexpr int VW = 16 / (int)sizeof(real);
+  using V = typename VecT<real, VW>::T;
+#pragma unroll
+  for (int v = 0; v < LEN / VW; ++v) {
+    const V x = reinterpret_cast<const V*>(p)[v];
+    const real* xs = reinterpret_cast<const real*>(&x);
+#pragma unroll
+    for (int e = 0; e < VW; ++e) out[v * VW + e] = xs[e];
+  }
+}
+
+template <typename real, int N, bool DUAL>
+__global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
+k_pipe(const __grid_constant__ StepArgs a) {
+  using O = Order<N>;
+  using Cfg = PipeCfg<real, N>;
+  using SM = PipeSmem<real, N>;
+  constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
+  constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL;
+  constexpr bool INPLACE = NT > 1;
+  constexpr int NTHREADS = G * NT * 32, NFLD = DUAL ? 2 : 1;
+  constexpr unsigned QBYTES = 4 * Np * 32 * sizeof(real), GBYTES = DG_NGEO * 32 * sizeof(real);
+  constexpr int RB = REC * (int)sizeof(real), CPB = RB % 16 == 0 ? 16 : (RB % 8 == 0 ? 8 : 4);
+  constexpr int CPW = CPB / (int)sizeof(real);
+  constexpr int FPW = (4 + NT - 1) / NT;                          // faces per warp
+
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  real* sD = reinterpret_cast<real*>(smem_raw);                   // [NT][Np][RL]
+  real* sL = sD + NT * Np * RL;                                   // [NT][NF][LL]
+  int* sF = reinterpret_cast<int*>(sL + NT * NF * LL);            // [NF]
+  int* sInv = sF + NF;                                            // [Np][3]
+  int* sP = sInv + 3 * Np;                                        // [kMaxPerm][Nfp]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::ops_bytes);   // [G][2]
+  real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + 256);
+
+  const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
+  real* grp = gbase + (size_t)g * SM::group_reals;
+  real* pen = grp + 2 * SM::stage_reals;                          // [2NF][32], later trace staging [4REC][32]
+  unsigned long long* full = bars + 2 * g;
+
+  {
+    const real* gD = static_cast<const real*>(a.ops2_D3Q);
+    const real* gL = static_cast<const real*>(a.ops2_LTQ);
+    for (int i = tid; i < NT * Np * RL; i += NTHREADS) sD[i] = gD[i];
+    for (int i = tid; i < NT * NF * LL; i += NTHREADS) sL[i] = gL[i];
+    for (int i = tid; i < NF; i += NTHREADS) sF[i] = a.ops.Fmask[i];
+    if (w == 0 && lane == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    load_face_tables<N>(a.ops, sInv, sP, NTHREADS);               // ends with __syncthreads
+  }
+  const real* myD = sD + (size_t)w * Np * RL;
+  const real* myL = sL + (size_t)w * NF * LL;
+
+  const int lo = a.blk0 + (int)(((long long)a.nblk * blockIdx.x) / gridDim.x);
+  const int hi = a.blk0 + (int)(((long long)a.nblk * (blockIdx.x + 1)) / gridDim.x);
+  const int nmine = (hi - lo - g + G - 1) / G;                    // blocks of this group
+  const int nitems = nmine > 0 ? nmine * NFLD : 0;
+  const real dir = (real)a.dir;
+  const int n0 = w * TO;
+
+  auto item_block = [&](int i) { return lo + g + (i / NFLD) * G; };
+  auto level_of = [&](int b) { int l = 0; while (b >= a.lv[l].blk_end) ++l; return l; };
+  auto load_codes = [&](int i, int (&code)[FPW]) {
+    const int b = item_block(i);
+#pragma unroll
+    for (int k = 0; k < FPW; ++k) {
+      const int f = w + k * NT;
+      code[k] = (f < 4 && i < nitems) ? a.nbr[((size_t)b * 4 + f) * 32 + lane] : -1;
+    }
+  };
+  // everything item i needs, into stage s: bulk copies by one lane, trace records by their consumer lanes
+  auto issue = [&](int i, int s, const int (&code)[FPW]) {
+    const int b = item_block(i), fi = i % NFLD, l = level_of(b);
+    const StepLevel& L = a.lv[l];
+    real* Q = grp + (size_t)s * SM::stage_reals;
+    if (w == 0 && lane == 0) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&full[s], 3 * QBYTES + GBYTES);
+      const size_t off = (size_t)b * (4 * Np * 32);
+      bulk_g2s(Q, static_cast<const real*>(a.q[fi]) + off, QBYTES, &full[s]);
+      bulk_g2s(Q + 4 * Np * 32, static_cast<const real*>(L.r1[fi]) + off, QBYTES, &full[s]);
+      bulk_g2s(Q + 8 * Np * 32, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[s]);
+      bulk_g2s(Q + 12 * Np * 32, static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES, &full[s]);
+    }
+    const int slot_lo = (l > 0 ? a.lv[l - 1].blk_end : 0) * 32, slot_hi = L.blk_end * 32;
+    const int lm = l > 0 ? l - 1 : 0, lp = l + 1 < a.nlevels ? l + 1 : l;
+    const real* qfm = static_cast<const real*>(a.lv[lm].qf_read[fi]);
+    const real* qf0 = static_cast<const real*>(L.qf_read[fi]);
+    const real* qfp = static_cast<const real*>(a.lv[lp].qf_read[fi]);
+    real* TR = Q + (12 * Np + DG_NGEO) * 32;
+#pragma unroll
+    for (int k = 0; k < FPW; ++k) {
+      const int f = w + k * NT, c = code[k];
+      if (f < 4 && c >= 0) {
+        const int s2 = c >> 2;
+        const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC;
+        real* dst = TR + ((size_t)f * 32 + lane) * REC;
+#pragma unroll
+        for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * CPW, src + v * CPW);
+      }
+    }
+  };
+
+  int codeA[FPW], codeB[FPW], codeC[FPW];
+  load_codes(0, codeA);
+  if (nitems > 0) issue(0, 0, codeA);
+  load_codes(1, codeB);
+  real simg[4][TO];                                               // imaging scalars of the source field
+
+#pragma unroll 1
+  for (int i = 0; i < nitems; ++i) {
+    const int s = i & 1, b = item_block(i), fi = i % NFLD, l = level_of(b);
+    const StepLevel& L = a.lv[l];
+    real* Q = grp + (size_t)s * SM::stage_reals;                  // [4Np][32]
+    const real* R1 = Q + 4 * Np * 32;
+    const real* R2 = Q + 8 * Np * 32;
+    const real* geo = Q + 12 * Np * 32 + lane;
+    const real* TR = Q + (12 * Np + DG_NGEO) * 32;
+    real* qg = static_cast<real*>(a.q[fi]);
+    const size_t base = (size_t)b * (4 * Np * 32) + lane;
+    const real c0 = (real)L.c[0], c1 = (real)L.c[1], c2 = (real)L.c[2];
+
+    group_sync<NT>(g);                          // the group has left the previous item (pen is free)
+    mbar_wait(&full[s], (unsigned)(i >> 1) & 1u);
+    cp_async_wait_all();
+    const real rc2 = geo[GEO_RC2 * 32], irho = geo[GEO_IRHO * 32];
+    real vold[3][TO];                                             // this tile's velocities before the in-place transform
+    if (INPLACE) {
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) {
+        const int n = n0 + nn < Np ? n0 + nn : Np - 1;
+        vold[0][nn] = Q[(Np + n) * 32 + lane]; vold[1][nn] = Q[(2 * Np + n) * 32 + lane]; vold[2][nn] = Q[(3 * Np + n) * 32 + lane];
+      }
+    }
+
+    // ---- penalties at the face nodes (Alg. 3, first half; eqs (11)-(12), readings Q2, Q4, Q6).  Branch-free
+    // inner loop: [[p]] = ap p- + ep_i, n.[[v]] = av (n.v)- + ev_i with per-face (ap, av) and exterior arrays
+    {
+      real* capt = fi == 0 ? static_cast<real*>(L.capture) : nullptr;
+      const real* repl = fi == 0 ? static_cast<const real*>(L.replay) : nullptr;
+#pragma unroll
+      for (int k = 0; k < FPW; ++k) {
+        const int f = w + k * NT;
+        if (f < 4) {
+          const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32],
+                     nz = geo[(GEO_FACE + 5 * f + 2) * 32], gs = geo[(GEO_FACE + 5 * f + 3) * 32],
+                     Zf = geo[(GEO_FACE + 5 * f + 4) * 32];
+          const int code = codeA[k];
+          const int bc = code >= 0 ? 0 : ((-1 - code) & 7), bpos = code >= 0 ? 0 : ((-1 - code) >> 3);
+          real ep[Nfp], ev[Nfp];
+          {
+            real rv[REC];
+            const real* src = TR + ((size_t)f * 32 + lane) * REC;
+            using V = typename VecT<real, CPW>::T;
+#pragma unroll
+            for (int v = 0; v < REC / CPW; ++v) {
+              const V x = reinterpret_cast<const V*>(src)[v];
+              const real* xs = reinterpret_cast<const real*>(&x);
+#pragma unroll
+              for (int e = 0; e < CPW; ++e) rv[v * CPW + e] = xs[e];
+            }
+#pragma unroll
+            for (int i2 = 0; i2 < Nfp; ++i2) {                       // interior: p+, n-.v+ = -(n+.v+) (reading Q6b)
+              ep[i2] = code >= 0 ? rv[i2] : (real)0;
+              ev[i2] = code >= 0 ? -rv[Nfp + i2] : (real)0;
+            }
+          }
+          // interior, absorbing, prescribed: -1, -1; free surface: -2, 0; rigid wall: 0, -2; padding slot: 0, 0
+          const real ap = (code >= 0 || bc == 2 || bc == 4) ? (real)-1 : (bc == 1 ? (real)-2 : (real)0);
+          const real av = (code >= 0 || bc == 2 || bc == 4) ? (real)-1 : (bc == 3 ? (real)-2 : (real)0);
+          const bool rep_lane = bc == 2 && repl != nullptr, ext_lane = bc == 4;
+          if (__any_sync(0xffffffffu, rep_lane || ext_lane)) {       // rare: exterior state from memory
+            if (rep_lane) {
+#pragma unroll
+              for (int i2 = 0; i2 < Nfp; ++i2) { ep[i2] = repl[(size_t)bpos * REC + i2]; ev[i2] = repl[(size_t)bpos * REC + Nfp + i2]; }
+            } else if (ext_lane) {
+              const real* ex = static_cast<const real*>(a.ext) + (size_t)bpos * Nfp * 2;
+#pragma unroll
+              for (int i2 = 0; i2 < Nfp; ++i2) { ep[i2] = ex[2 * i2]; ev[i2] = ex[2 * i2 + 1]; }
+            }
+          }
+          const bool cap_lane = bc == 2 && capt != nullptr;
+          const bool cap_any = __any_sync(0xffffffffu, cap_lane);
+          const real kp = rc2 * (real)0.5 * gs, kv = irho * (real)0.5 * gs, diZ = dir / Zf, dZ = dir * Zf;
+#pragma unroll
+          for (int i2 = 0; i2 < Nfp; ++i2) {
+            const int j = f * Nfp + i2, n = sF[j];
+            const real pm = Q[n * 32 + lane];
+            const real nvm = nx * Q[(Np + n) * 32 + lane] + ny * Q[(2 * Np + n) * 32 + lane] + nz * Q[(3 * Np + n) * 32 + lane];
+            if (cap_any && cap_lane) { capt[(size_t)bpos * REC + i2] = pm; capt[(size_t)bpos * REC + Nfp + i2] = nvm; }
+            const real dp = ap * pm + ep[i2], dnv = av * nvm + ev[i2];
+            pen[j * 32 + lane] = kp * (dnv - diZ * dp);
+            pen[(NF + j) * 32 + lane] = kv * (dp - dZ * dnv);
+          }
+        }
+      }
+    }
+    const real g00 = geo[0 * 32], g01 = geo[1 * 32], g02 = geo[2 * 32], g10 = geo[3 * 32], g11 = geo[4 * 32],
+               g12 = geo[5 * 32], g20 = geo[6 * 32], g21 = geo[7 * 32], g22 = geo[8 * 32];
+    group_sync<NT>(g);                          // penalties done; every warp has left the previous item
+    // ---- the other stage is free now: fetch the next item; codes two items ahead
+    if (i + 1 < nitems) issue(i + 1, s ^ 1, codeB);
+    load_codes(i + 2, codeC);
+    const int wp = a.wperm[(size_t)b * 32 + lane];
+    const int pi = a.pt_index[fi] ? a.pt_index[fi][(size_t)b * 32 + lane] : -1;
+    if (INPLACE) {                              // v -> (U.Gr, U.Gs, U.Gt) once per block (Alg. 2)
+      for (int m = w; m < Np; m += NT) {
+        const real vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
+        Q[(Np + m) * 32 + lane] = g00 * vx + g10 * vy + g20 * vz;
+        Q[(2 * Np + m) * 32 + lane] = g01 * vx + g11 * vy + g21 * vz;
+        Q[(3 * Np + m) * 32 + lane] = g02 * vx + g12 * vy + g22 * vz;
+      }
+      group_sync<NT>(g);
+    }
+
+    // ---- volume (eqs (13)-(14), Alg. 2)
+    real rp[TO], rx[TO], ry[TO], rz[TO];
+    {
+      real aD[TO], aR[TO], aS[TO], aT[TO];
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) { aD[nn] = 0; aR[nn] = 0; aS[nn] = 0; aT[nn] = 0; }
+#pragma unroll 4
+      for (int m = 0; m < Np; ++m) {
+        const real p = Q[m * 32 + lane];
+        real ur, us, ut;
+        if (INPLACE) {
+          ur = Q[(Np + m) * 32 + lane]; us = Q[(2 * Np + m) * 32 + lane]; ut = Q[(3 * Np + m) * 32 + lane];
+        } else {
+          const real vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
+          ur = g00 * vx + g10 * vy + g20 * vz; us = g01 * vx + g11 * vy + g21 * vz; ut = g02 * vx + g12 * vy + g22 * vz;
+        }
+        real d[RL];
+        load_packed<real, RL>(myD + m * RL, d);
+#pragma unroll
+        for (int nn = 0; nn < TO; ++nn) {
+          aD[nn] = fma(d[nn], ur, aD[nn]); aD[nn] = fma(d[TO + nn], us, aD[nn]); aD[nn] = fma(d[2 * TO + nn], ut, aD[nn]);
+          aR[nn] = fma(d[nn], p, aR[nn]); aS[nn] = fma(d[TO + nn], p, aS[nn]); aT[nn] = fma(d[2 * TO + nn], p, aT[nn]);
+        }
+      }
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) {
+        rp[nn] = -rc2 * aD[nn];
+        rx[nn] = -irho * (g00 * aR[nn] + g01 * aS[nn] + g02 * aT[nn]);
+        ry[nn] = -irho * (g10 * aR[nn] + g11 * aS[nn] + g12 * aT[nn]);
+        rz[nn] = -irho * (g20 * aR[nn] + g21 * aS[nn] + g22 * aT[nn]);
+      }
+    }
+    group_sync<NT>(g);                          // every warp has read Q: the update may overwrite its tile's nodes
+    // ---- surface (Alg. 3, second half)
+#pragma unroll 1
+    for (int f = 0; f < 4; ++f) {
+      real av[TO];
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
+#pragma unroll
+      for (int i2 = 0; i2 < Nfp; ++i2) {
+        const int j = f * Nfp + i2;
+        const real Pp = pen[j * 32 + lane], Pv = pen[(NF + j) * 32 + lane];
+        real lv[LL];
+        load_packed<real, LL>(myL + j * LL, lv);
+#pragma unroll
+        for (int nn = 0; nn < TO; ++nn) { rp[nn] -= lv[nn] * Pp; av[nn] += lv[nn] * Pv; }
+      }
+      const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
+    }
+
+    // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
+    const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);
+    {
+      constexpr bool FULL = TO * NT == Np;                          // no padded outputs: no guards
+      real* r0p = static_cast<real*>(L.r0[fi]) + base + (size_t)n0 * 32;
+      real* qp = qg + base + (size_t)n0 * 32;
+      const real* ptv = static_cast<const real*>(a.pt_val[fi]) + (size_t)(pi < 0 ? 0 : pi) * Np;
+      const real pts = (real)a.pt_scale[fi];
+      const bool imaging = DUAL && L.image_on;
+      const real Z = (imaging && a.characteristic) ? geo[GEO_Z * 32] : (real)0;
+      const real ex = (real)a.e[0], ey = (real)a.e[1], ez = (real)a.e[2];
+      const real sgn = fi == 0 ? (real)-1 : (real)1;      // q_S^- = p - Z e.v ; q_R^+ = p + Z e.v  (eq (8))
+      const real dts = (real)L.dts, adts = dts < 0 ? -dts : dts;
+      real* imgp = static_cast<real*>(a.image) + ((size_t)b * Np + n0) * 32 + lane;
+      const real d0 = (real)L.d[0], d1 = (real)L.d[1], d2 = (real)L.d[2];
+      real* Qt = Q + n0 * 32 + lane;
+      const real* R1t = R1 + n0 * 32 + lane;
+      const real* R2t = R2 + n0 * 32 + lane;
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) {
+        if (FULL || n0 + nn < Np) {
+          real r0v[4] = {rp[nn], rx[nn], ry[nn], rz[nn]}, qo[4], h1[4], h2[4], v[4];
+          if (pi >= 0) r0v[0] += pts * ptv[n0 + nn];
+          qo[0] = Qt[nn * 32];
+#pragma unroll
+          for (int fld = 1; fld < 4; ++fld) qo[fld] = INPLACE ? vold[fld - 1][nn] : Qt[(fld * Np + nn) * 32];
+#pragma unroll
+          for (int fld = 0; fld < 4; ++fld) { h1[fld] = R1t[(fld * Np + nn) * 32]; h2[fld] = R2t[(fld * Np + nn) * 32]; }
+#pragma unroll
+          for (int fld = 0; fld < 4; ++fld) {
+            v[fld] = qo[fld] + (c0 * r0v[fld] + c1 * h1[fld] + c2 * h2[fld]);
+            r0p[(fld * Np + nn) * 32] = r0v[fld];
+            qp[(fld * Np + nn) * 32] = v[fld];
+            Qt[(fld * Np + nn) * 32] = v[fld];
+          }
+          if (imaging) {
+            const real A0 = qo[0] + sgn * Z * (ex * qo[1] + ey * qo[2] + ez * qo[3]);
+            const real A1 = r0v[0] + sgn * Z * (ex * r0v[1] + ey * r0v[2] + ez * r0v[3]);
+            const real A2 = h1[0] + sgn * Z * (ex * h1[1] + ey * h1[2] + ez * h1[3]);
+            const real A3 = h2[0] + sgn * Z * (ex * h2[1] + ey * h2[2] + ez * h2[3]);
+            if (fi == 0) {
+              simg[0][nn] = A0; simg[1][nn] = A1; simg[2][nn] = A2; simg[3][nn] = A3;
+            } else {
+              const real S0 = simg[0][nn];
+              const real rA[3] = {simg[1][nn], simg[2][nn], simg[3][nn]};
+              const real rB[3] = {A1, A2, A3};
+              real acc = S0 * A0;
+#pragma unroll
+              for (int k = 0; k < 3; ++k) {
+                acc += dts * (real)L.abar[k] * (S0 * rB[k] + A0 * rA[k]);
+#pragma unroll
+                for (int k2 = 0; k2 < 3; ++k2) acc += dts * dts * (real)L.C[3 * k + k2] * rA[k] * rB[k2];
+              }
+              imgp[nn * 32] += adts * acc;
+            }
+          }
+          // value at the half step (19) = new value + sum_s d_s r_s; kept for the second trace pass
+          if (need_half) {
+#pragma unroll
+            for (int fld = 0; fld < 4; ++fld) v[fld] += d0 * r0v[fld] + d1 * h1[fld] + d2 * h2[fld];
+          }
+          rp[nn] = v[0]; rx[nn] = v[1]; ry[nn] = v[2]; rz[nn] = v[3];
+        }
+      }
+    }
+
+    // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
+    // per face from Q, placed at the reader's positions (permutation table), staged in pen as [row][lane]
+#pragma unroll 1
+    for (int pass = 0; pass < (need_half ? 2 : 1); ++pass) {
+      if (pass == 1) {
+        group_sync<NT>(g);                      // pass 0 has gathered from Q
+        constexpr bool FULL = TO * NT == Np;
+        real* Qt = Q + n0 * 32 + lane;
+#pragma unroll
+        for (int nn = 0; nn < TO; ++nn)
+          if (FULL || n0 + nn < Np) {
+            Qt[nn * 32] = rp[nn]; Qt[(Np + nn) * 32] = rx[nn]; Qt[(2 * Np + nn) * 32] = ry[nn]; Qt[(3 * Np + nn) * 32] = rz[nn];
+          }
+      }
+      group_sync<NT>(g);                        // Q holds the values of this pass; pen is free
+#pragma unroll
+      for (int k = 0; k < FPW; ++k) {
+        const int f = w + k * NT;
+        if (f < 4) {
+          const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
+          const int* prow = sP + ((wp >> (8 * f)) & 255) * Nfp;
+          real* st = pen + f * REC * 32 + lane;
+#pragma unroll
+          for (int i2 = 0; i2 < Nfp; ++i2) {
+            const int n = sF[f * Nfp + i2], pos = prow[i2];
+            st[pos * 32] = Q[n * 32 + lane];
+            st[(Nfp + pos) * 32] = nx * Q[(Np + n) * 32 + lane] + ny * Q[(2 * Np + n) * 32 + lane] + nz * Q[(3 * Np + n) * 32 + lane];
+          }
+        }
+      }
+      group_sync<NT>(g);
+      {
+        constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
+        using V = typename VecT<real, VS>::T;
+        real* dst = static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + ((size_t)b * 32 + lane) * ROWS;
+        for (int v = w; v < NV; v += NT) {
+          V x;
+          real* xs = reinterpret_cast<real*>(&x);
+#pragma unroll
+          for (int e = 0; e < VS; ++e) xs[e] = pen[(v * VS + e) * 32 + lane];
+          reinterpret_cast<V*>(dst)[v] = x;
+        }
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < FPW; ++k) { codeA[k] = codeB[k]; codeB[k] = codeC[k]; }
+  }
+}
+
+}  // namespace dgrtm
