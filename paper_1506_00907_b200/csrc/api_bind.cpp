@@ -59,8 +59,20 @@ void upload_tables(dg_ctx* c) {
           }
           for (int j = 0; j < NF; ++j) LTQ[((size_t)w * NF + j) * LL + nn] = re.LIFT[(size_t)n * NF + j];
         }
-      upload_real(c, c->d_D3Q, D3Q.data(), D3Q.size());
-      upload_real(c, c->d_LTQ, LTQ.data(), LTQ.size());
+      // the kernel's table image: reals (device precision) then Fmask and the permutation table
+      std::vector<char> blob(c->kt->pipe_blob_bytes, 0);
+      size_t off = 0;
+      auto put_reals = [&](const std::vector<double>& v) {
+        for (double x : v) {
+          if (c->precision == 64) { std::memcpy(&blob[off], &x, 8); off += 8; }
+          else { const float f = (float)x; std::memcpy(&blob[off], &f, 4); off += 4; }
+        }
+      };
+      put_reals(D3Q); put_reals(LTQ);
+      std::memcpy(&blob[off], re.Fmask.data(), (size_t)NF * 4); off += (size_t)NF * 4;
+      if (off + m.ptab.size() * 4 > blob.size()) throw ApiError(DG_ERR_UNSUPPORTED, "too many distinct face permutations");
+      std::memcpy(&blob[off], m.ptab.data(), m.ptab.size() * 4);
+      upload_raw(c, c->d_D3Q, blob.data(), blob.size());
     }
   }
   upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);

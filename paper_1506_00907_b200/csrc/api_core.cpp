@@ -342,9 +342,8 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
     const int npad = c->kt ? c->kt->step_npad : Np;
     c->d_D3P = cv.take((size_t)3 * Np * npad * rs);
     c->d_LTP = cv.take((size_t)NF * npad * rs);
-    const int nt = c->kt ? c->kt->pipe_NT : 0;
-    c->d_D3Q = cv.take((size_t)std::max(1, nt * Np * (c->kt ? c->kt->pipe_RL : 0)) * rs);
-    c->d_LTQ = cv.take((size_t)std::max(1, nt * NF * (c->kt ? c->kt->pipe_LL : 0)) * rs);
+    c->d_D3Q = cv.take(std::max<size_t>(16, c->kt ? c->kt->pipe_blob_bytes : 0));
+    c->d_LTQ = nullptr;
   }
   c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks);
   c->d_pt_src = (int*)cv.take((size_t)md.nslots * 4);

@@ -126,11 +126,12 @@ template <typename real> KernelTable make_table(int precision) {
   t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
   t.capture = Launch<real>::capture; t.init = Launch<real>::init;
-  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0;
+  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0;
   if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
     t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
     t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;
     t.pipe_RL = PipeSmem<real, N>::RL; t.pipe_LL = PipeSmem<real, N>::LL;
+    t.pipe_blob_bytes = PipeSmem<real, N>::ops_bytes;
   }
   t.step = Launch<real>::step; t.step2 = Launch<real>::step2; t.step_npad = StepSmem<real, N, false>::NPAD;
   return t;

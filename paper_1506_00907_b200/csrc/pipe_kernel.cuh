@@ -18,7 +18,7 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #define DG_P3_NT 4
-#define DG_P3_G 2
+#define DG_P3_G 3
 #endif
 template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G; };
 
@@ -29,11 +29,13 @@ template <typename real, int N> struct PipeSmem {
   static constexpr int RL = (3 * C::TO + VW - 1) / VW * VW;        // packed derivative row
   static constexpr int LL = (C::TO + VW - 1) / VW * VW;            // packed lift row
   static constexpr size_t ops_reals = (size_t)C::NT * O::Np * RL + (size_t)C::NT * O::NF * LL;
-  static constexpr size_t tab_ints = O::NF + 3 * O::Np + UpdSmem<N>::kMaxPerm * O::Nfp;
+  static constexpr size_t tab_ints = O::NF + UpdSmem<N>::kMaxPerm * O::Nfp;     // Fmask, permutation table
   static constexpr size_t ops_bytes = (ops_reals * sizeof(real) + tab_ints * sizeof(int) + 127) / 128 * 128;
-  // one stage: q, r1, r2 [4Np][32] each, factors [DG_NGEO][32], neighbour records [4][32][REC]
-  static constexpr size_t stage_reals = (size_t)(12 * O::Np + DG_NGEO + 4 * O::REC) * 32;
-  static constexpr size_t group_reals = 2 * stage_reals + (size_t)2 * O::NF * 32;      // + penalties / staging
+  // two stages of q [4Np][32] + factors [DG_NGEO][32]; single buffers: r1, r2 [4Np][32] each (fetched after
+  // the previous item's update), neighbour records [4][32][REC] (fetched after the previous item's
+  // penalties), penalties / trace staging [2NF][32]
+  static constexpr size_t stage_reals = (size_t)(4 * O::Np + DG_NGEO) * 32;
+  static constexpr size_t group_reals = 2 * stage_reals + (size_t)(8 * O::Np + 4 * O::REC + 2 * O::NF) * 32;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
   static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
@@ -79,25 +81,28 @@ k_pipe(const __grid_constant__ StepArgs a) {
   real* sD = reinterpret_cast<real*>(smem_raw);                   // [NT][Np][RL]
   real* sL = sD + NT * Np * RL;                                   // [NT][NF][LL]
   int* sF = reinterpret_cast<int*>(sL + NT * NF * LL);            // [NF]
-  int* sInv = sF + NF;                                            // [Np][3]
-  int* sP = sInv + 3 * Np;                                        // [kMaxPerm][Nfp]
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::ops_bytes);   // [G][2]
+  int* sP = sF + NF;                                              // [kMaxPerm][Nfp]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::ops_bytes);   // [G][3], tables
   real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + 256);
 
   const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
   real* grp = gbase + (size_t)g * SM::group_reals;
-  real* pen = grp + 2 * SM::stage_reals;                          // [2NF][32], later trace staging [4REC][32]
-  unsigned long long* full = bars + 2 * g;
+  real* R1 = grp + 2 * SM::stage_reals;                           // [4Np][32]
+  real* R2 = R1 + 4 * Np * 32;                                    // [4Np][32]
+  real* TR = R2 + 4 * Np * 32;                                    // [4][32][REC]
+  real* pen = TR + 4 * REC * 32;                                  // [2NF][32], later trace staging [4REC][32]
+  unsigned long long* full = bars + 3 * g;                        // [0], [1]: q stages; [2]: r1, r2
+  unsigned long long* tabbar = bars + 3 * G;
 
-  {
-    const real* gD = static_cast<const real*>(a.ops2_D3Q);
-    const real* gL = static_cast<const real*>(a.ops2_LTQ);
-    for (int i = tid; i < NT * Np * RL; i += NTHREADS) sD[i] = gD[i];
-    for (int i = tid; i < NT * NF * LL; i += NTHREADS) sL[i] = gL[i];
-    for (int i = tid; i < NF; i += NTHREADS) sF[i] = a.ops.Fmask[i];
-    if (w == 0 && lane == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    load_face_tables<N>(a.ops, sInv, sP, NTHREADS);               // ends with __syncthreads
+  {  // operator tables + Fmask + permutation table: one blob, laid out on the host exactly as here
+    if (tid == 0) {
+      mbar_init(tabbar, 1);
+      for (int x = 0; x < 3 * G; ++x) mbar_init(&bars[x], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      mbar_expect_tx(tabbar, (unsigned)SM::ops_bytes);
+      bulk_g2s(smem_raw, a.ops2_D3Q, (unsigned)SM::ops_bytes, tabbar);
+    }
+    __syncthreads();
   }
   const real* myD = sD + (size_t)w * Np * RL;
   const real* myL = sL + (size_t)w * NF * LL;
@@ -120,25 +125,33 @@ k_pipe(const __grid_constant__ StepArgs a) {
     }
   };
   // everything item i needs, into stage s: bulk copies by one lane, trace records by their consumer lanes
+  // the two older right-hand sides of item i (single buffer: call after the previous item's update)
+  auto issue_r = [&](int i) {
+    if (w == 0 && lane == 0) {
+      const int b = item_block(i), fi = i % NFLD;
+      const StepLevel& L = a.lv[level_of(b)];
+      const size_t off = (size_t)b * (4 * Np * 32);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(&full[2], 2 * QBYTES);
+      bulk_g2s(R1, static_cast<const real*>(L.r1[fi]) + off, QBYTES, &full[2]);
+      bulk_g2s(R2, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[2]);
+    }
+  };
   auto issue = [&](int i, int s, const int (&code)[FPW]) {
     const int b = item_block(i), fi = i % NFLD, l = level_of(b);
     const StepLevel& L = a.lv[l];
     real* Q = grp + (size_t)s * SM::stage_reals;
     if (w == 0 && lane == 0) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(&full[s], 3 * QBYTES + GBYTES);
-      const size_t off = (size_t)b * (4 * Np * 32);
-      bulk_g2s(Q, static_cast<const real*>(a.q[fi]) + off, QBYTES, &full[s]);
-      bulk_g2s(Q + 4 * Np * 32, static_cast<const real*>(L.r1[fi]) + off, QBYTES, &full[s]);
-      bulk_g2s(Q + 8 * Np * 32, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[s]);
-      bulk_g2s(Q + 12 * Np * 32, static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES, &full[s]);
+      mbar_expect_tx(&full[s], QBYTES + GBYTES);
+      bulk_g2s(Q, static_cast<const real*>(a.q[fi]) + (size_t)b * (4 * Np * 32), QBYTES, &full[s]);
+      bulk_g2s(Q + 4 * Np * 32, static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES, &full[s]);
     }
     const int slot_lo = (l > 0 ? a.lv[l - 1].blk_end : 0) * 32, slot_hi = L.blk_end * 32;
     const int lm = l > 0 ? l - 1 : 0, lp = l + 1 < a.nlevels ? l + 1 : l;
     const real* qfm = static_cast<const real*>(a.lv[lm].qf_read[fi]);
     const real* qf0 = static_cast<const real*>(L.qf_read[fi]);
     const real* qfp = static_cast<const real*>(a.lv[lp].qf_read[fi]);
-    real* TR = Q + (12 * Np + DG_NGEO) * 32;
 #pragma unroll
     for (int k = 0; k < FPW; ++k) {
       const int f = w + k * NT, c = code[k];
@@ -154,8 +167,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
   int codeA[FPW], codeB[FPW], codeC[FPW];
   load_codes(0, codeA);
-  if (nitems > 0) issue(0, 0, codeA);
+  if (nitems > 0) { issue(0, 0, codeA); issue_r(0); }
   load_codes(1, codeB);
+  mbar_wait(tabbar, 0);
   real simg[4][TO];                                               // imaging scalars of the source field
 
 #pragma unroll 1
@@ -163,10 +177,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     const int s = i & 1, b = item_block(i), fi = i % NFLD, l = level_of(b);
     const StepLevel& L = a.lv[l];
     real* Q = grp + (size_t)s * SM::stage_reals;                  // [4Np][32]
-    const real* R1 = Q + 4 * Np * 32;
-    const real* R2 = Q + 8 * Np * 32;
-    const real* geo = Q + 12 * Np * 32 + lane;
-    const real* TR = Q + (12 * Np + DG_NGEO) * 32;
+    const real* geo = Q + 4 * Np * 32 + lane;
     real* qg = static_cast<real*>(a.q[fi]);
     const size_t base = (size_t)b * (4 * Np * 32) + lane;
     const real c0 = (real)L.c[0], c1 = (real)L.c[1], c2 = (real)L.c[2];
@@ -319,6 +330,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
     const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);
+    mbar_wait(&full[2], (unsigned)i & 1u);
     {
       constexpr bool FULL = TO * NT == Np;                          // no padded outputs: no guards
       real* r0p = static_cast<real*>(L.r0[fi]) + base + (size_t)n0 * 32;
@@ -383,6 +395,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
       }
     }
 
+    group_sync<NT>(g);                          // Q holds the new values; r1, r2 are consumed
+    if (i + 1 < nitems) issue_r(i + 1);
     // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
     // per face from Q, placed at the reader's positions (permutation table), staged in pen as [row][lane]
 #pragma unroll 1
@@ -397,7 +411,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
             Qt[nn * 32] = rp[nn]; Qt[(Np + nn) * 32] = rx[nn]; Qt[(2 * Np + nn) * 32] = ry[nn]; Qt[(3 * Np + nn) * 32] = rz[nn];
           }
       }
-      group_sync<NT>(g);                        // Q holds the values of this pass; pen is free
+      if (pass == 1) group_sync<NT>(g);         // Q holds the values of this pass; pen is free
 #pragma unroll
       for (int k = 0; k < FPW; ++k) {
         const int f = w + k * NT;
