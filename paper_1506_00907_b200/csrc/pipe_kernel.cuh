@@ -35,7 +35,10 @@ template <typename real, int N> struct PipeSmem {
   // the previous item's update), neighbour records [4][32][REC] (fetched after the previous item's
   // penalties), penalties / trace staging [2NF][32]
   static constexpr size_t stage_reals = (size_t)(4 * O::Np + DG_NGEO) * 32;
-  static constexpr size_t group_reals = 2 * stage_reals + (size_t)(8 * O::Np + 4 * O::REC + 2 * O::NF) * 32;
+  // penalties: [face][Pp | Pv][ceil(Nfp / VW)][lane][VW] (one vector load = VW face nodes of my element)
+  static constexpr int PV = (O::Nfp + VW - 1) / VW;               // vectors per face and penalty kind
+  static constexpr size_t pen_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
+  static constexpr size_t group_reals = 2 * stage_reals + (size_t)(8 * O::Np + 4 * O::REC) * 32 + pen_reals;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
   static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
@@ -69,7 +72,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   using Cfg = PipeCfg<real, N>;
   using SM = PipeSmem<real, N>;
   constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
-  constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL;
+  constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
   constexpr bool INPLACE = NT > 1;
   constexpr int NTHREADS = G * NT * 32, NFLD = DUAL ? 2 : 1;
   constexpr unsigned QBYTES = 4 * Np * 32 * sizeof(real), GBYTES = DG_NGEO * 32 * sizeof(real);
@@ -244,6 +247,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
           const bool cap_lane = bc == 2 && capt != nullptr;
           const bool cap_any = __any_sync(0xffffffffu, cap_lane);
           const real kp = rc2 * (real)0.5 * gs, kv = irho * (real)0.5 * gs, diZ = dir / Zf, dZ = dir * Zf;
+          real Pp[PV * VW], Pv[PV * VW];
+#pragma unroll
+          for (int i2 = Nfp; i2 < PV * VW; ++i2) { Pp[i2] = 0; Pv[i2] = 0; }
 #pragma unroll
           for (int i2 = 0; i2 < Nfp; ++i2) {
             const int j = f * Nfp + i2, n = sF[j];
@@ -251,8 +257,18 @@ k_pipe(const __grid_constant__ StepArgs a) {
             const real nvm = nx * Q[(Np + n) * 32 + lane] + ny * Q[(2 * Np + n) * 32 + lane] + nz * Q[(3 * Np + n) * 32 + lane];
             if (cap_any && cap_lane) { capt[(size_t)bpos * REC + i2] = pm; capt[(size_t)bpos * REC + Nfp + i2] = nvm; }
             const real dp = ap * pm + ep[i2], dnv = av * nvm + ev[i2];
-            pen[j * 32 + lane] = kp * (dnv - diZ * dp);
-            pen[(NF + j) * 32 + lane] = kv * (dp - dZ * dnv);
+            Pp[i2] = kp * (dnv - diZ * dp);
+            Pv[i2] = kv * (dp - dZ * dnv);
+          }
+          {
+            using V = typename VecT<real, VW>::T;
+            V* dstp = reinterpret_cast<V*>(pen) + ((size_t)(f * 2 + 0) * PV) * 32 + lane;
+            V* dstv = reinterpret_cast<V*>(pen) + ((size_t)(f * 2 + 1) * PV) * 32 + lane;
+#pragma unroll
+            for (int v = 0; v < PV; ++v) {
+              dstp[v * 32] = *reinterpret_cast<const V*>(&Pp[v * VW]);
+              dstv[v * 32] = *reinterpret_cast<const V*>(&Pv[v * VW]);
+            }
           }
         }
       }
@@ -314,10 +330,21 @@ k_pipe(const __grid_constant__ StepArgs a) {
       real av[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
+      real Ppv[PV * VW], Pvv[PV * VW];
+      {
+        using V = typename VecT<real, VW>::T;
+        const V* srcp = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 0) * PV) * 32 + lane;
+        const V* srcv = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 1) * PV) * 32 + lane;
+#pragma unroll
+        for (int v = 0; v < PV; ++v) {
+          *reinterpret_cast<V*>(&Ppv[v * VW]) = srcp[v * 32];
+          *reinterpret_cast<V*>(&Pvv[v * VW]) = srcv[v * 32];
+        }
+      }
 #pragma unroll
       for (int i2 = 0; i2 < Nfp; ++i2) {
         const int j = f * Nfp + i2;
-        const real Pp = pen[j * 32 + lane], Pv = pen[(NF + j) * 32 + lane];
+        const real Pp = Ppv[i2], Pv = Pvv[i2];
         real lv[LL];
         load_packed<real, LL>(myL + j * LL, lv);
 #pragma unroll
