@@ -22,6 +22,20 @@ inline int persistent_grid(int nblk, int per_sm) {
   return nblk < cap ? nblk : cap;
 }
 
+// launch with programmatic stream serialization: the kernel's prologue may overlap the previous kernel's
+// tail; the kernel itself waits (griddepcontrol.wait) before touching data the previous launch wrote
+template <typename K>
+void launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_t s, const StepArgs& a) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)threads);
+  cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kernel, a);
+}
+
 template <typename real> struct Launch {
   static int occ_rhs, occ_upd, occ_rk, occ_img;
 
@@ -91,12 +105,12 @@ template <typename real> struct Launch {
   static void pipe(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    k_pipe<real, N, false><<<a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s>>>(a);
+    launch_pdl(k_pipe<real, N, false>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void pipe2(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    k_pipe<real, N, true><<<a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s>>>(a);
+    launch_pdl(k_pipe<real, N, true>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
   static void record(const PointArgs& a, cudaStream_t s) {

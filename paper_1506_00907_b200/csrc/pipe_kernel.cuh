@@ -169,6 +169,10 @@ k_pipe(const __grid_constant__ StepArgs a) {
   };
 
   int codeA[FPW], codeB[FPW], codeC[FPW];
+  // programmatic dependent launch: everything above overlapped the tail of the previous launch on the
+  // stream; from here on its results (q, right-hand sides, traces) are read
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   load_codes(0, codeA);
   if (nitems > 0) { issue(0, 0, codeA); issue_r(0); }
   load_codes(1, codeB);
