@@ -73,6 +73,9 @@ void upload_tables(dg_ctx* c) {
       if (off + m.ptab.size() * 4 > blob.size()) throw ApiError(DG_ERR_UNSUPPORTED, "too many distinct face permutations");
       std::memcpy(&blob[off], m.ptab.data(), m.ptab.size() * 4);
       upload_raw(c, c->d_D3Q, blob.data(), blob.size());
+      const int ce = c->kt->pipe_set_const(blob.data(), c->stream);
+      if (ce != 0) throw ApiError(DG_ERR_CUDA, std::string("constant tables: ") + cudaGetErrorString((cudaError_t)ce));
+      sync_stream(c);
     }
   }
   upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);

@@ -158,7 +158,8 @@ struct KernelTable {
   void (*pipe)(const StepArgs&, cudaStream_t);
   void (*pipe2)(const StepArgs&, cudaStream_t);
   int pipe_TO, pipe_NT, pipe_RL, pipe_LL;
-  size_t pipe_blob_bytes;                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
+  size_t pipe_blob_bytes;
+  int (*pipe_set_const)(const void* blob_host, cudaStream_t);   // operator part of the blob -> constant memory                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
   int (*init)();           // sets shared-memory attributes; returns cudaError
 };
 

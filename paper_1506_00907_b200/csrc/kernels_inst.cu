@@ -112,6 +112,14 @@ template <typename real> struct Launch {
     using C = PipeCfg<real, N>;
     launch_pdl(k_pipe<real, N, true>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
+  static int pipe_set_const(const void* blob_host, cudaStream_t s) {
+    if constexpr (PipeCfg<real, N>::enabled) {
+      const size_t n = PipeSmem<real, N>::ops_reals * sizeof(real);
+      if constexpr (sizeof(real) == 4) return (int)cudaMemcpyToSymbolAsync(c_pipe_ops_f, blob_host, n, 0, cudaMemcpyHostToDevice, s);
+      else return (int)cudaMemcpyToSymbolAsync(c_pipe_ops_d, blob_host, n, 0, cudaMemcpyHostToDevice, s);
+    }
+    return 0;
+  }
   static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
   static void record(const PointArgs& a, cudaStream_t s) {
     if (a.nr <= 0) return;
@@ -140,12 +148,12 @@ template <typename real> KernelTable make_table(int precision) {
   t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
   t.capture = Launch<real>::capture; t.init = Launch<real>::init;
-  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0;
+  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0; t.pipe_set_const = nullptr;
   if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
     t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
     t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;
     t.pipe_RL = PipeSmem<real, N>::RL; t.pipe_LL = PipeSmem<real, N>::LL;
-    t.pipe_blob_bytes = PipeSmem<real, N>::ops_bytes;
+    t.pipe_blob_bytes = PipeSmem<real, N>::ops_bytes; t.pipe_set_const = Launch<real>::pipe_set_const;
   }
   t.step = Launch<real>::step; t.step2 = Launch<real>::step2; t.step_npad = StepSmem<real, N, false>::NPAD;
   return t;

@@ -14,13 +14,21 @@
 
 namespace dgrtm {
 
-template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1; };
+// TO outputs per warp, NT warps per block, G groups per CTA, QS = stages of the q ring (2: fetched one item
+// ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1; };
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #define DG_P3_NT 4
 #define DG_P3_G 3
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G; };
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2; };
+#ifndef DG_P4_TO
+#define DG_P4_TO 5
+#define DG_P4_NT 7
+#define DG_P4_G 2
+#endif
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1; };
 
 template <typename real, int N> struct PipeSmem {
   using O = Order<N>;
@@ -38,7 +46,7 @@ template <typename real, int N> struct PipeSmem {
   // penalties: [face][Pp | Pv][ceil(Nfp / VW)][lane][VW] (one vector load = VW face nodes of my element)
   static constexpr int PV = (O::Nfp + VW - 1) / VW;               // vectors per face and penalty kind
   static constexpr size_t pen_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
-  static constexpr size_t group_reals = 2 * stage_reals + (size_t)(8 * O::Np + 4 * O::REC) * 32 + pen_reals;
+  static constexpr size_t group_reals = C::QS * stage_reals + (size_t)(8 * O::Np + 4 * O::REC) * 32 + pen_reals;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
   static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
@@ -65,6 +73,104 @@ __device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&o
   }
 }
 
+// ---- operator tables in constant memory: with the tile index and all loop indices known at compile time
+// every operator entry becomes a c[bank][offset] operand of its FFMA / DFMA: no shared-memory traffic and
+// no load instruction for the operators (one table per translation unit = per order).
+// MEASURED (B200, N = 3 fp32, cfg2): ptxas turns the entries into LDCU.128 -> uniform registers -> FFMA R,R,UR,R;
+// the 10 KB table streams through the small constant cache and the step slows from 66 to 112 us (N = 4: 3.1x
+// slower).  Kept as a compile-time option (-DDG_PIPE_COPS=1), off by default; see DESIGN.md.
+#ifndef DG_PIPE_COPS
+#define DG_PIPE_COPS 0
+#endif
+#ifdef DG_ORDER
+__constant__ float c_pipe_ops_f[PipeCfg<float, DG_ORDER>::enabled ? PipeSmem<float, DG_ORDER>::ops_reals : 1];
+__constant__ double c_pipe_ops_d[PipeCfg<double, DG_ORDER>::enabled ? PipeSmem<double, DG_ORDER>::ops_reals : 1];
+template <typename real> struct PipeConst;
+template <> struct PipeConst<float> { static __device__ __forceinline__ const float* ops() { return c_pipe_ops_f; } };
+template <> struct PipeConst<double> { static __device__ __forceinline__ const double* ops() { return c_pipe_ops_d; } };
+
+// volume + surface of output tile TILE (= warp w of the group) with constant-bank operators
+template <typename real, int N, int TILE>
+__device__ __forceinline__ void pipe_tile_const(const real* __restrict__ Q, const real* __restrict__ pen, const real* __restrict__ geo,
+                                                int lane, int g, real rc2, real irho, const real (&gm)[9],
+                                                real (&rp)[PipeCfg<real, N>::TO], real (&rx)[PipeCfg<real, N>::TO],
+                                                real (&ry)[PipeCfg<real, N>::TO], real (&rz)[PipeCfg<real, N>::TO]) {
+  using O = Order<N>;
+  using Cfg = PipeCfg<real, N>;
+  using SM = PipeSmem<real, N>;
+  constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, TO = Cfg::TO, NT = Cfg::NT, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
+  constexpr bool INPLACE = NT > 1;
+  const real* cD = PipeConst<real>::ops() + (size_t)TILE * Np * RL;
+  const real* cL = PipeConst<real>::ops() + (size_t)NT * Np * RL + (size_t)TILE * NF * LL;
+  real aD[TO], aR[TO], aS[TO], aT[TO];
+#pragma unroll
+  for (int nn = 0; nn < TO; ++nn) { aD[nn] = 0; aR[nn] = 0; aS[nn] = 0; aT[nn] = 0; }
+#pragma unroll
+  for (int m = 0; m < Np; ++m) {
+    const real p = Q[m * 32 + lane];
+    real ur, us, ut;
+    if (INPLACE) {
+      ur = Q[(Np + m) * 32 + lane]; us = Q[(2 * Np + m) * 32 + lane]; ut = Q[(3 * Np + m) * 32 + lane];
+    } else {
+      const real vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
+      ur = gm[0] * vx + gm[3] * vy + gm[6] * vz; us = gm[1] * vx + gm[4] * vy + gm[7] * vz; ut = gm[2] * vx + gm[5] * vy + gm[8] * vz;
+    }
+#pragma unroll
+    for (int nn = 0; nn < TO; ++nn) {
+      const real dr = cD[m * RL + nn], ds = cD[m * RL + TO + nn], dt = cD[m * RL + 2 * TO + nn];
+      aD[nn] = fma(dr, ur, aD[nn]); aD[nn] = fma(ds, us, aD[nn]); aD[nn] = fma(dt, ut, aD[nn]);
+      aR[nn] = fma(dr, p, aR[nn]); aS[nn] = fma(ds, p, aS[nn]); aT[nn] = fma(dt, p, aT[nn]);
+    }
+  }
+#pragma unroll
+  for (int nn = 0; nn < TO; ++nn) {
+    rp[nn] = -rc2 * aD[nn];
+    rx[nn] = -irho * (gm[0] * aR[nn] + gm[1] * aS[nn] + gm[2] * aT[nn]);
+    ry[nn] = -irho * (gm[3] * aR[nn] + gm[4] * aS[nn] + gm[5] * aT[nn]);
+    rz[nn] = -irho * (gm[6] * aR[nn] + gm[7] * aS[nn] + gm[8] * aT[nn]);
+  }
+  group_sync<NT>(g);                          // every warp has read Q: the update may overwrite its tile's nodes
+#pragma unroll
+  for (int f = 0; f < 4; ++f) {
+    real av[TO];
+#pragma unroll
+    for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
+    real Ppv[PV * VW], Pvv[PV * VW];
+    {
+      using V = typename VecT<real, VW>::T;
+      const V* srcp = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 0) * PV) * 32 + lane;
+      const V* srcv = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 1) * PV) * 32 + lane;
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        *reinterpret_cast<V*>(&Ppv[v * VW]) = srcp[v * 32];
+        *reinterpret_cast<V*>(&Pvv[v * VW]) = srcv[v * 32];
+      }
+    }
+#pragma unroll
+    for (int i2 = 0; i2 < Nfp; ++i2) {
+      const int j = f * Nfp + i2;
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) {
+        const real lv = cL[j * LL + nn];
+        rp[nn] = fma(-lv, Ppv[i2], rp[nn]); av[nn] = fma(lv, Pvv[i2], av[nn]);
+      }
+    }
+    const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
+#pragma unroll
+    for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
+  }
+}
+template <typename real, int N, int TILE>
+__device__ __forceinline__ void pipe_tile_dispatch(int w, const real* Q, const real* pen, const real* geo, int lane, int g, real rc2,
+                                                   real irho, const real (&gm)[9], real (&rp)[PipeCfg<real, N>::TO],
+                                                   real (&rx)[PipeCfg<real, N>::TO], real (&ry)[PipeCfg<real, N>::TO],
+                                                   real (&rz)[PipeCfg<real, N>::TO]) {
+  if (w == TILE) pipe_tile_const<real, N, TILE>(Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
+  else if constexpr (TILE + 1 < PipeCfg<real, N>::NT)
+    pipe_tile_dispatch<real, N, TILE + 1>(w, Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
+}
+#endif  // DG_ORDER
+
 template <typename real, int N, bool DUAL>
 __global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
 k_pipe(const __grid_constant__ StepArgs a) {
@@ -74,6 +180,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
   constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
   constexpr bool INPLACE = NT > 1;
+  constexpr int QS = Cfg::QS;
   constexpr int NTHREADS = G * NT * 32, NFLD = DUAL ? 2 : 1;
   constexpr unsigned QBYTES = 4 * Np * 32 * sizeof(real), GBYTES = DG_NGEO * 32 * sizeof(real);
   constexpr int RB = REC * (int)sizeof(real), CPB = RB % 16 == 0 ? 16 : (RB % 8 == 0 ? 8 : 4);
@@ -90,7 +197,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
   const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
   real* grp = gbase + (size_t)g * SM::group_reals;
-  real* R1 = grp + 2 * SM::stage_reals;                           // [4Np][32]
+  real* R1 = grp + QS * SM::stage_reals;                          // [4Np][32]
   real* R2 = R1 + 4 * Np * 32;                                    // [4Np][32]
   real* TR = R2 + 4 * Np * 32;                                    // [4][32][REC]
   real* pen = TR + 4 * REC * 32;                                  // [2NF][32], later trace staging [4REC][32]
@@ -140,16 +247,28 @@ k_pipe(const __grid_constant__ StepArgs a) {
       bulk_g2s(R2, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[2]);
     }
   };
-  auto issue = [&](int i, int s, const int (&code)[FPW]) {
-    const int b = item_block(i), fi = i % NFLD, l = level_of(b);
-    const StepLevel& L = a.lv[l];
-    real* Q = grp + (size_t)s * SM::stage_reals;
+  // q and the factors of item i into stage s (bulk copies by one lane)
+  auto issue_q = [&](int i, int s) {
     if (w == 0 && lane == 0) {
+      const int b = item_block(i), fi = i % NFLD;
+      real* Q = grp + (size_t)s * SM::stage_reals;
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_expect_tx(&full[s], QBYTES + GBYTES);
       bulk_g2s(Q, static_cast<const real*>(a.q[fi]) + (size_t)b * (4 * Np * 32), QBYTES, &full[s]);
       bulk_g2s(Q + 4 * Np * 32, static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES, &full[s]);
     }
+  };
+  auto prefetch_q = [&](int i) {
+    if (w == 0 && lane == 0) {
+      const int b = item_block(i), fi = i % NFLD;
+      bulk_prefetch_l2(static_cast<const real*>(a.q[fi]) + (size_t)b * (4 * Np * 32), QBYTES);
+      bulk_prefetch_l2(static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES);
+    }
+  };
+  // the neighbours' trace records of item i (per-lane cp.async by their consumer lanes)
+  auto issue_tr = [&](int i, const int (&code)[FPW]) {
+    const int b = item_block(i), fi = i % NFLD, l = level_of(b);
+    const StepLevel& L = a.lv[l];
     const int slot_lo = (l > 0 ? a.lv[l - 1].blk_end : 0) * 32, slot_hi = L.blk_end * 32;
     const int lm = l > 0 ? l - 1 : 0, lp = l + 1 < a.nlevels ? l + 1 : l;
     const real* qfm = static_cast<const real*>(a.lv[lm].qf_read[fi]);
@@ -174,14 +293,14 @@ k_pipe(const __grid_constant__ StepArgs a) {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
   load_codes(0, codeA);
-  if (nitems > 0) { issue(0, 0, codeA); issue_r(0); }
+  if (nitems > 0) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
   real simg[4][TO];                                               // imaging scalars of the source field
 
 #pragma unroll 1
   for (int i = 0; i < nitems; ++i) {
-    const int s = i & 1, b = item_block(i), fi = i % NFLD, l = level_of(b);
+    const int s = QS == 2 ? (i & 1) : 0, b = item_block(i), fi = i % NFLD, l = level_of(b);
     const StepLevel& L = a.lv[l];
     real* Q = grp + (size_t)s * SM::stage_reals;                  // [4Np][32]
     const real* geo = Q + 4 * Np * 32 + lane;
@@ -190,7 +309,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
     const real c0 = (real)L.c[0], c1 = (real)L.c[1], c2 = (real)L.c[2];
 
     group_sync<NT>(g);                          // the group has left the previous item (pen is free)
-    mbar_wait(&full[s], (unsigned)(i >> 1) & 1u);
+    if (QS == 1 && i > 0) issue_q(i, 0);
+    mbar_wait(&full[s], (unsigned)(QS == 2 ? (i >> 1) : i) & 1u);
     cp_async_wait_all();
     const real rc2 = geo[GEO_RC2 * 32], irho = geo[GEO_IRHO * 32];
     real vold[3][TO];                                             // this tile's velocities before the in-place transform
@@ -281,7 +401,10 @@ k_pipe(const __grid_constant__ StepArgs a) {
                g12 = geo[5 * 32], g20 = geo[6 * 32], g21 = geo[7 * 32], g22 = geo[8 * 32];
     group_sync<NT>(g);                          // penalties done; every warp has left the previous item
     // ---- the other stage is free now: fetch the next item; codes two items ahead
-    if (i + 1 < nitems) issue(i + 1, s ^ 1, codeB);
+    if (i + 1 < nitems) {
+      if (QS == 2) issue_q(i + 1, s ^ 1); else prefetch_q(i + 1);
+      issue_tr(i + 1, codeB);
+    }
     load_codes(i + 2, codeC);
     const int wp = a.wperm[(size_t)b * 32 + lane];
     const int pi = a.pt_index[fi] ? a.pt_index[fi][(size_t)b * 32 + lane] : -1;
@@ -297,11 +420,21 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- volume (eqs (13)-(14), Alg. 2)
     real rp[TO], rx[TO], ry[TO], rz[TO];
+#if DG_PIPE_COPS
+    {
+      const real gm[9] = {g00, g01, g02, g10, g11, g12, g20, g21, g22};
+      pipe_tile_dispatch<real, N, 0>(w, Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
+    }
+#else
     {
       real aD[TO], aR[TO], aS[TO], aT[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { aD[nn] = 0; aR[nn] = 0; aS[nn] = 0; aT[nn] = 0; }
-#pragma unroll 4
+#ifndef DG_PIPE_UNROLL_M
+#define DG_PIPE_UNROLL_M 5
+#endif
+      constexpr int UM = DG_PIPE_UNROLL_M;
+#pragma unroll UM
       for (int m = 0; m < Np; ++m) {
         const real p = Q[m * 32 + lane];
         real ur, us, ut;
@@ -358,6 +491,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
     }
+#endif
 
     // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
     const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);
