@@ -69,7 +69,7 @@ def build(force=False, orders=(1, 2, 3, 4, 5, 6), verbose=False):
         obj = os.path.join(OBJ, name.replace(".cpp", ".o"))
         objs.append(obj)
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
-            jobs.append(["g++", "-std=c++17", "-O2", "-fPIC", "-Wall", "-I", os.path.join(CUDA_HOME, "include"),
+            jobs.append(["g++", "-std=c++17", "-O2", "-fPIC", "-Wall", "-pthread", "-I", os.path.join(CUDA_HOME, "include"),
                          "-c", src, "-o", obj])
     logs = []
     if jobs:
@@ -79,7 +79,7 @@ def build(force=False, orders=(1, 2, 3, 4, 5, 6), verbose=False):
         for lg in logs:
             sys.stdout.write(lg)
     if jobs or force or not os.path.exists(LIB):
-        _run([NVCC, "-shared", *ARCH, "-o", LIB, *objs, "-lquadmath"])
+        _run([NVCC, "-shared", *ARCH, "-o", LIB, *objs, "-lquadmath", "-lpthread"])
     return LIB
 
 

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <mutex>
+#include <thread>
 
 #include "ctx.h"
 
@@ -128,30 +129,63 @@ void download_real(dg_ctx* c, double* dst, const void* src, size_t n) {
   for (size_t i = 0; i < n; ++i) dst[i] = (double)tmp[i];
 }
 
-void fields_to_device(dg_ctx* c, char* dq, const double* q) {
-  const int Np = c->Np;
-  const int64_t ns = c->model.nslots;
-  std::vector<double> tmp((size_t)ns * 4 * Np, 0.0);
-  for (int64_t s = 0; s < ns; ++s) {
-    const int64_t k = c->model.elem_of[s];
-    if (k < 0) continue;
-    const int64_t b = s >> 5, lane = s & 31;
-    for (int x = 0; x < 4 * Np; ++x) tmp[((size_t)b * 4 * Np + x) * 32 + lane] = q[(size_t)k * 4 * Np + x];
+// user order q[K][4][Np] <-> device [block][4Np][32], converted to / from the device precision in one pass,
+// slots split over host threads (the e2e path: dg_set_state / dg_get_fields)
+namespace {
+template <typename F> void parallel_slots(int64_t ns, F body) {
+  unsigned nt = std::thread::hardware_concurrency();
+  nt = nt == 0 ? 1 : (nt > 16 ? 16 : nt);
+  if (ns < 4096) nt = 1;
+  std::vector<std::thread> th;
+  const int64_t nb = (ns + 31) / 32, per = (nb + nt - 1) / nt;
+  for (unsigned t = 0; t < nt; ++t) {
+    const int64_t b0 = t * per, b1 = std::min<int64_t>(nb, b0 + per);
+    if (b0 >= b1) break;
+    th.emplace_back([=] { body(b0 * 32, std::min<int64_t>(ns, b1 * 32)); });
   }
-  upload_real(c, dq, tmp.data(), tmp.size());
+  for (auto& x : th) x.join();
+}
+template <typename real> void pack_fields(const dg_ctx* c, real* out, const double* q) {
+  const int W = 4 * c->Np;
+  parallel_slots(c->model.nslots, [&](int64_t s0, int64_t s1) {
+    for (int64_t s = s0; s < s1; ++s) {
+      const int64_t k = c->model.elem_of[s], b = s >> 5, lane = s & 31;
+      real* o = out + (size_t)b * W * 32 + lane;
+      if (k < 0) { for (int x = 0; x < W; ++x) o[(size_t)x * 32] = 0; continue; }
+      const double* in = q + (size_t)k * W;
+      for (int x = 0; x < W; ++x) o[(size_t)x * 32] = (real)in[x];
+    }
+  });
+}
+template <typename real> void unpack_fields(const dg_ctx* c, double* q, const real* in) {
+  const int W = 4 * c->Np;
+  parallel_slots(c->model.nslots, [&](int64_t s0, int64_t s1) {
+    for (int64_t s = s0; s < s1; ++s) {
+      const int64_t k = c->model.elem_of[s], b = s >> 5, lane = s & 31;
+      if (k < 0) continue;
+      const real* i = in + (size_t)b * W * 32 + lane;
+      double* o = q + (size_t)k * W;
+      for (int x = 0; x < W; ++x) o[x] = (double)i[(size_t)x * 32];
+    }
+  });
+}
+}  // namespace
+
+void fields_to_device(dg_ctx* c, char* dq, const double* q) {
+  const size_t n = (size_t)c->model.nslots * 4 * c->Np;
+  std::vector<char> tmp(n * c->rs);
+  if (c->precision == 64) pack_fields(c, reinterpret_cast<double*>(tmp.data()), q);
+  else pack_fields(c, reinterpret_cast<float*>(tmp.data()), q);
+  upload_raw(c, dq, tmp.data(), tmp.size());
 }
 
 void fields_from_device(dg_ctx* c, double* q, const char* dq) {
-  const int Np = c->Np;
-  const int64_t ns = c->model.nslots;
-  std::vector<double> tmp((size_t)ns * 4 * Np);
-  download_real(c, tmp.data(), dq, tmp.size());
-  for (int64_t s = 0; s < ns; ++s) {
-    const int64_t k = c->model.elem_of[s];
-    if (k < 0) continue;
-    const int64_t b = s >> 5, lane = s & 31;
-    for (int x = 0; x < 4 * Np; ++x) q[(size_t)k * 4 * Np + x] = tmp[((size_t)b * 4 * Np + x) * 32 + lane];
-  }
+  const size_t n = (size_t)c->model.nslots * 4 * c->Np;
+  std::vector<char> tmp(n * c->rs);
+  cuda_check(cudaMemcpyAsync(tmp.data(), dq, tmp.size(), cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
+  sync_stream(c);
+  if (c->precision == 64) unpack_fields(c, q, reinterpret_cast<const double*>(tmp.data()));
+  else unpack_fields(c, q, reinterpret_cast<const float*>(tmp.data()));
 }
 
 void clear_field(dg_ctx* c, Field& F) {

@@ -247,6 +247,36 @@ def test_cfg4_rtm_shot(precision, nlevels, imaging):
     g.close()
 
 
+@pytest.mark.parametrize("precision,N,nlevels", [(32, 4, 1), (32, 4, 3), (64, 3, 3), (32, 5, 1), (64, 4, 1), (32, 1, 3)])
+def test_rtm_shot_other_orders(precision, N, nlevels):
+    """The two-wavefield kernels of the other orders / precisions (several warps per element block, padded
+    output tiles, imaging scalars in registers, shared or global memory): forward + backward + image."""
+    nsteps = 16
+    if nlevels == 1:
+        cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=N, nsteps=nsteps, n_receivers_side=3)
+    else:
+        cfg = make_config("cfg3_lts", hexes=(5, 5, 6), N=N, nsteps=nsteps)
+        gx = np.linspace(0.4, 2.6, 3)
+        cfg["receivers"] = np.array([[x + 0.013, y + 0.007, 0.06] for x in gx for y in gx])
+        cfg["updir"] = np.array([0.0, 0.0, -1.0])
+    cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
+    o = make_oracle(cfg)
+    g = make_gpu(cfg, precision, history_steps=nsteps)
+    tol = TOL[precision]
+    data_g = g.rtm_forward_shot(nsteps)
+    data_o, hist, qT = o.rtm_forward(nsteps)
+    assert np.abs(data_o).max() > 0
+    assert rel_l2(data_g, data_o) < tol
+    assert rel_l2(g.rtm_get_fields(0), qT) < tol
+    g.rtm_backward_shot(nsteps, data_o, updir=cfg["updir"])
+    I_o, FS, FR = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], nglobal_total=nsteps)
+    assert rel_l2(g.rtm_get_fields(1), FS.q) < tol * 3
+    assert rel_l2(g.rtm_get_fields(2), FR.q) < tol * 3
+    assert np.abs(I_o).max() > 0
+    assert rel_l2(g.rtm_image_read(), I_o) < (1e-4 if precision == 32 else 1e-10)
+    g.close()
+
+
 def test_rtm_first_image_step():
     cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=2, nsteps=40, n_receivers_side=3)
     cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
@@ -278,6 +308,30 @@ def test_cfg5_orders(N, precision):
     o.run_mrab([F], nsteps, 0.0, 1, source_on=(True,))
     assert np.linalg.norm(F.q) > 0
     assert rel_l2(g.dg_get_fields(), F.q) < TOL[precision]
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# full BASELINE.json sizes in the launch configuration bench.py times (every CTA, every group of the
+# pipelined kernel, ragged chunks): a few steps from a random state, every element compared
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,nsteps", [("cfg2_two_layer", 5), ("cfg4_rtm", 2)])
+def test_full_size_short_run(name, nsteps):
+    cfg = make_config(name)
+    cfg["receivers"] = None
+    o = make_oracle(cfg)
+    g = make_gpu(cfg, 32)
+    assert g.K == {"cfg2_two_layer": 98304, "cfg4_rtm": 786432}[name]
+    q0 = random_state(o.K, o.Np, 11)
+    g.dg_set_state(q0)
+    g.dg_step(nsteps)
+    F = o.new_field(q0)
+    o.run_mrab([F], nsteps, 0.0, 1, source_on=(True,))
+    qg = g.dg_get_fields()
+    assert rel_l2(qg, F.q) < TOL[32]
+    # element by element: no block of the mesh may be off (a mis-scheduled block would not show in a global norm)
+    err = np.sqrt(((qg - F.q) ** 2).sum(axis=(1, 2)) / (F.q ** 2).sum(axis=(1, 2)))
+    assert err.max() < 20 * TOL[32]
     g.close()
 
 
