@@ -157,6 +157,21 @@ def make_ctx(cfg, device, history_steps=0):
     return g
 
 
+def max_over_ranks(sec, dist, device):
+    """Time of a multi-rank run = the slowest rank's device time (dist: an initialised torch.distributed)."""
+    if dist is None:
+        return sec
+    import torch
+    t = torch.tensor([sec], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(dof_per_rank_step, steps, world, sec):
+    """Replicas only: every rank advances the same workload; value = all ranks' DOF-updates / slowest time."""
+    return world * dof_per_rank_step * steps / sec
+
+
 def timed_steps(g, torch, T, K, W, dist, device):
     """W warm-up + K timed bench steps of dg_step(T) on the bound stream; returns max-over-ranks seconds."""
     for _ in range(W):
@@ -175,11 +190,7 @@ def timed_steps(g, torch, T, K, W, dist, device):
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize(device)
-    sec = e0.elapsed_time(e1) * 1e-3
-    if dist is not None:
-        t = torch.tensor([sec], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec = float(t.item())
+    sec = max_over_ranks(e0.elapsed_time(e1) * 1e-3, dist, device)
     return sec, g.dg_get_launch_count() - n0
 
 
@@ -398,7 +409,7 @@ def run_ours(args):
     sampler.start()
     sec, launches = timed_steps(g, torch, T, K, W, dist, device)
     clocks = sampler.stop()
-    value = world * dof_step * T * K / sec
+    value = whole_job_value(dof_step * T, K, world, sec)
 
     # roofline of the dominant kernel: separate pass, one event pair per launch
     roof, ker, oth = profile_kernels(g, T, max(1, min(K, 3)), dof_step // (4 * Np), Np, Nfp, rs, peak, peak_src,
@@ -409,10 +420,7 @@ def run_ours(args):
     q0 = 1e-3 * rng.standard_normal((g.K, 4, Np))
     Ke = max(1, min(K, 5))
     sec_e, _ = run_e2e(g, torch, T, Ke, q0, device)
-    if dist is not None:
-        t = torch.tensor([sec_e], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec_e = float(t.item())
+    sec_e = max_over_ranks(sec_e, dist, device)
     field_bytes = int(g.K) * 4 * Np * rs
     e2e = {"value": world * dof_step * T * Ke / sec_e, "unit": UNIT, "h2d_bytes_per_step": field_bytes,
            "d2h_bytes_per_step": field_bytes, "ms_per_step": 1e3 * sec_e / Ke,
@@ -447,7 +455,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, N, precision); None until captured
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {("cfg2_two_layer", 3, 32): 196859904}      # profiles/r1b_fused_pipeline.md (147.65 MB read + 49.21 MB written)
 
 
 if __name__ == "__main__":
