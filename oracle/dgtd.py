@@ -17,6 +17,10 @@ PAPER.md = /root/reference/PAPER.md.  Implemented, in the paper's notation:
     (readings Q1, Q1b).
   * LSERK4 (not in the paper; BASELINE.json config 1 only, reading Q8).
 
+Parity unpinned (no value of the paper or of mathematics fixes them; only GPU-vs-oracle agreement and the
+properties tested in tests/test_oracle_scheme.py hold): the AB start-up ramp by AB1, AB2 (reading Q7), the
+reconstructed source wavefield and the image values at the configurations.
+
 Array conventions: q[k, field, n] with field 0 = p, 1..3 = v_x, v_y, v_z; traces qf[k, f, i, 0] = p,
 qf[k, f, i, 1] = n.v (outward normal of the owner); levels: 0 = coarsest (paper's
 l = 1), L-1 = finest.
