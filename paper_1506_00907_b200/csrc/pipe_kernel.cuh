@@ -16,19 +16,31 @@ namespace dgrtm {
 
 // TO outputs per warp, NT warps per block, G groups per CTA, QS = stages of the q ring (2: fetched one item
 // ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
-template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1; };
+// RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: read from global in the
+// update phase after an L2 prefetch (saves 8Np rows of shared memory per group: more groups per SM)
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1; };
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #define DG_P3_NT 4
 #define DG_P3_G 3
+#define DG_P3_RS 1
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2; };
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2, RS = DG_P3_RS; };
 #ifndef DG_P4_TO
-#define DG_P4_TO 5
-#define DG_P4_NT 7
-#define DG_P4_G 2
+#define DG_P4_TO 7
+#define DG_P4_NT 5
+#define DG_P4_G 3
+#define DG_P4_RS 0
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS; };
+#ifndef DG_D3_TO
+#define DG_D3_TO 5
+#define DG_D3_NT 4
+#define DG_D3_G 3
+#endif
+#ifndef DG_D3_OFF
+template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0; };
+#endif
 
 template <typename real, int N> struct PipeSmem {
   using O = Order<N>;
@@ -46,7 +58,7 @@ template <typename real, int N> struct PipeSmem {
   // penalties: [face][Pp | Pv][ceil(Nfp / VW)][lane][VW] (one vector load = VW face nodes of my element)
   static constexpr int PV = (O::Nfp + VW - 1) / VW;               // vectors per face and penalty kind
   static constexpr size_t pen_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
-  static constexpr size_t group_reals = C::QS * stage_reals + (size_t)(8 * O::Np + 4 * O::REC) * 32 + pen_reals;
+  static constexpr size_t group_reals = C::QS * stage_reals + (size_t)(C::RS * 8 * O::Np + 4 * O::REC) * 32 + pen_reals;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
   static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
@@ -180,7 +192,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
   constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
   constexpr bool INPLACE = NT > 1;
-  constexpr int QS = Cfg::QS;
+  constexpr int QS = Cfg::QS, RS = Cfg::RS;
   constexpr int NTHREADS = G * NT * 32, NFLD = DUAL ? 2 : 1;
   constexpr unsigned QBYTES = 4 * Np * 32 * sizeof(real), GBYTES = DG_NGEO * 32 * sizeof(real);
   constexpr int RB = REC * (int)sizeof(real), CPB = RB % 16 == 0 ? 16 : (RB % 8 == 0 ? 8 : 4);
@@ -198,8 +210,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
   const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
   real* grp = gbase + (size_t)g * SM::group_reals;
   real* R1 = grp + QS * SM::stage_reals;                          // [4Np][32]
-  real* R2 = R1 + 4 * Np * 32;                                    // [4Np][32]
-  real* TR = R2 + 4 * Np * 32;                                    // [4][32][REC]
+  real* R2 = R1 + RS * 4 * Np * 32;                               // [4Np][32]
+  real* TR = R2 + RS * 4 * Np * 32;                               // [4][32][REC]
   real* pen = TR + 4 * REC * 32;                                  // [2NF][32], later trace staging [4REC][32]
   unsigned long long* full = bars + 3 * g;                        // [0], [1]: q stages; [2]: r1, r2
   unsigned long long* tabbar = bars + 3 * G;
@@ -241,10 +253,15 @@ k_pipe(const __grid_constant__ StepArgs a) {
       const int b = item_block(i), fi = i % NFLD;
       const StepLevel& L = a.lv[level_of(b)];
       const size_t off = (size_t)b * (4 * Np * 32);
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(&full[2], 2 * QBYTES);
-      bulk_g2s(R1, static_cast<const real*>(L.r1[fi]) + off, QBYTES, &full[2]);
-      bulk_g2s(R2, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[2]);
+      if (RS) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&full[2], 2 * QBYTES);
+        bulk_g2s(R1, static_cast<const real*>(L.r1[fi]) + off, QBYTES, &full[2]);
+        bulk_g2s(R2, static_cast<const real*>(L.r2[fi]) + off, QBYTES, &full[2]);
+      } else {
+        bulk_prefetch_l2(static_cast<const real*>(L.r1[fi]) + off, QBYTES);
+        bulk_prefetch_l2(static_cast<const real*>(L.r2[fi]) + off, QBYTES);
+      }
     }
   };
   // q and the factors of item i into stage s (bulk copies by one lane)
@@ -495,7 +512,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
     const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);
-    mbar_wait(&full[2], (unsigned)i & 1u);
+    if (RS) mbar_wait(&full[2], (unsigned)i & 1u);
     {
       constexpr bool FULL = TO * NT == Np;                          // no padded outputs: no guards
       real* r0p = static_cast<real*>(L.r0[fi]) + base + (size_t)n0 * 32;
@@ -510,8 +527,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
       real* imgp = static_cast<real*>(a.image) + ((size_t)b * Np + n0) * 32 + lane;
       const real d0 = (real)L.d[0], d1 = (real)L.d[1], d2 = (real)L.d[2];
       real* Qt = Q + n0 * 32 + lane;
-      const real* R1t = R1 + n0 * 32 + lane;
-      const real* R2t = R2 + n0 * 32 + lane;
+      const real* R1t = RS ? R1 + n0 * 32 + lane : static_cast<const real*>(L.r1[fi]) + base + (size_t)n0 * 32;
+      const real* R2t = RS ? R2 + n0 * 32 + lane : static_cast<const real*>(L.r2[fi]) + base + (size_t)n0 * 32;
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) {
         if (FULL || n0 + nn < Np) {
