@@ -313,6 +313,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
   if (nitems > 0) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
+  int fofs[FPW][Nfp];                                             // own-trace offsets of this warp's faces in Q
+#pragma unroll
+  for (int k = 0; k < FPW; ++k)
+#pragma unroll
+    for (int i2 = 0; i2 < Nfp; ++i2) fofs[k][i2] = (w + k * NT < 4 ? sF[(w + k * NT) * Nfp + i2] : 0) * 32 + lane;
   real simg[4][TO];                                               // imaging scalars of the source field
 
 #pragma unroll 1
@@ -393,9 +398,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
           for (int i2 = Nfp; i2 < PV * VW; ++i2) { Pp[i2] = 0; Pv[i2] = 0; }
 #pragma unroll
           for (int i2 = 0; i2 < Nfp; ++i2) {
-            const int j = f * Nfp + i2, n = sF[j];
-            const real pm = Q[n * 32 + lane];
-            const real nvm = nx * Q[(Np + n) * 32 + lane] + ny * Q[(2 * Np + n) * 32 + lane] + nz * Q[(3 * Np + n) * 32 + lane];
+            const int o = fofs[k][i2];
+            const real pm = Q[o];
+            const real nvm = nx * Q[Np * 32 + o] + ny * Q[2 * Np * 32 + o] + nz * Q[3 * Np * 32 + o];
             if (cap_any && cap_lane) { capt[(size_t)bpos * REC + i2] = pm; capt[(size_t)bpos * REC + Nfp + i2] = nvm; }
             const real dp = ap * pm + ep[i2], dnv = av * nvm + ev[i2];
             Pp[i2] = kp * (dnv - diZ * dp);
@@ -603,9 +608,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
           real* st = pen + f * REC * 32 + lane;
 #pragma unroll
           for (int i2 = 0; i2 < Nfp; ++i2) {
-            const int n = sF[f * Nfp + i2], pos = prow[i2];
-            st[pos * 32] = Q[n * 32 + lane];
-            st[(Nfp + pos) * 32] = nx * Q[(Np + n) * 32 + lane] + ny * Q[(2 * Np + n) * 32 + lane] + nz * Q[(3 * Np + n) * 32 + lane];
+            const int o = fofs[k][i2], pos = prow[i2];
+            st[pos * 32] = Q[o];
+            st[(Nfp + pos) * 32] = nx * Q[Np * 32 + o] + ny * Q[2 * Np * 32 + o] + nz * Q[3 * Np * 32 + o];
           }
         }
       }
