@@ -18,28 +18,30 @@ namespace dgrtm {
 // ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
 // RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: read from global in the
 // update phase after an L2 prefetch (saves 8Np rows of shared memory per group: more groups per SM)
-template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1; };
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1; };
+// UG = 1: velocities -> U.G once per block, in place in shared memory; 0: every warp forms U.G on the fly
+// (9 more FMAs per input node and warp, two shared-memory passes and one barrier fewer)
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #define DG_P3_NT 4
 #define DG_P3_G 3
 #define DG_P3_RS 1
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2, RS = DG_P3_RS; };
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2, RS = DG_P3_RS, UG = 0; };
 #ifndef DG_P4_TO
 #define DG_P4_TO 7
 #define DG_P4_NT 5
 #define DG_P4_G 3
 #define DG_P4_RS 0
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = 1; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
 #define DG_D3_G 3
 #endif
 #ifndef DG_D3_OFF
-template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0; };
+template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0; };
 #endif
 
 template <typename real, int N> struct PipeSmem {
@@ -111,7 +113,7 @@ __device__ __forceinline__ void pipe_tile_const(const real* __restrict__ Q, cons
   using Cfg = PipeCfg<real, N>;
   using SM = PipeSmem<real, N>;
   constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, TO = Cfg::TO, NT = Cfg::NT, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
-  constexpr bool INPLACE = NT > 1;
+  constexpr bool INPLACE = NT > 1 && Cfg::UG;
   const real* cD = PipeConst<real>::ops() + (size_t)TILE * Np * RL;
   const real* cL = PipeConst<real>::ops() + (size_t)NT * Np * RL + (size_t)TILE * NF * LL;
   real aD[TO], aR[TO], aS[TO], aT[TO];
@@ -191,7 +193,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   using SM = PipeSmem<real, N>;
   constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
   constexpr int TO = Cfg::TO, NT = Cfg::NT, G = Cfg::G, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
-  constexpr bool INPLACE = NT > 1;
+  constexpr bool INPLACE = NT > 1 && Cfg::UG;
   constexpr int QS = Cfg::QS, RS = Cfg::RS;
   constexpr int NTHREADS = G * NT * 32, NFLD = DUAL ? 2 : 1;
   constexpr unsigned QBYTES = 4 * Np * 32 * sizeof(real), GBYTES = DG_NGEO * 32 * sizeof(real);
