@@ -77,6 +77,37 @@ void upload_tables(dg_ctx* c) {
       if (ce != 0) throw ApiError(DG_ERR_CUDA, std::string("constant tables: ") + cudaGetErrorString((cudaError_t)ce));
       sync_stream(c);
     }
+    if (c->kt->tc) {     // tensor-core kernel: B tables in the canonical K-major no-swizzle layout, split hi / lo (TF32)
+      const int K1 = c->kt->tc_K1, K2 = c->kt->tc_K2, NN = c->kt->tc_NN;
+      auto tf32 = [](float x) {             // round to nearest even at 10 mantissa bits
+        uint32_t u; std::memcpy(&u, &x, 4);
+        u = (u + 0x0FFFu + ((u >> 13) & 1u)) & 0xFFFFE000u;
+        float y; std::memcpy(&y, &u, 4); return y;
+      };
+      auto idx = [NN](int kap, int n) { return (size_t)(kap / 8) * (8 * NN) + ((size_t)(((kap % 8) / 4) * NN + n) * 4 + (kap % 4)); };
+      std::vector<float> B1h((size_t)K1 * NN, 0.f), B1l(B1h), B2h((size_t)K2 * NN, 0.f), B2l(B2h);
+      for (int j = 0; j < 3; ++j)
+        for (int mm = 0; mm < Np; ++mm)
+          for (int n = 0; n < Np; ++n) {
+            const std::vector<double>& D = j == 0 ? re.Dr : (j == 1 ? re.Ds : re.Dt);
+            const double v = D[(size_t)n * Np + mm];
+            const float h = tf32((float)v);
+            B1h[idx(j * Np + mm, n)] = h; B1l[idx(j * Np + mm, n)] = tf32((float)(v - (double)h));
+          }
+      for (int j = 0; j < NF; ++j)
+        for (int n = 0; n < Np; ++n) {
+          const double v = re.LIFT[(size_t)n * NF + j];
+          const float h = tf32((float)v);
+          B2h[idx(j, n)] = h; B2l[idx(j, n)] = tf32((float)(v - (double)h));
+        }
+      std::vector<char> blob(c->kt->tc_blob_bytes, 0);
+      size_t off = 0;
+      for (const std::vector<float>* t : {&B1h, &B1l, &B2h, &B2l}) { std::memcpy(&blob[off], t->data(), t->size() * 4); off += t->size() * 4; }
+      std::memcpy(&blob[off], re.Fmask.data(), (size_t)NF * 4); off += (size_t)NF * 4;
+      if (off + m.ptab.size() * 4 > blob.size()) throw ApiError(DG_ERR_UNSUPPORTED, "too many distinct face permutations");
+      std::memcpy(&blob[off], m.ptab.data(), m.ptab.size() * 4);
+      upload_raw(c, c->d_LTQ, blob.data(), blob.size());
+    }
   }
   upload_raw(c, const_cast<int*>(c->ops.Fmask), re.Fmask.data(), (size_t)NF * 4);
   upload_raw(c, const_cast<int*>(c->ops.ptab), m.ptab.data(), m.ptab.size() * 4);

@@ -258,7 +258,7 @@ int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, co
     c->kt = get_kernel_table(N, precision);
     for (int l = 0; l < kMaxLevels; ++l) { c->d_coarse[l] = nullptr; c->d_stored[l] = nullptr; c->rec[l] = nullptr; }
     c->F.reset_history(); c->R.reset_history();
-    if (const char* k = std::getenv("DGRTM_KERNEL")) c->use_pipe = std::string(k) != "step";
+    if (const char* k = std::getenv("DGRTM_KERNEL")) { c->use_pipe = std::string(k) != "step"; c->use_tc = std::string(k) == "tc"; }
   } catch (const std::exception& e) {
     g_create_error = e.what();
     delete c;
@@ -377,7 +377,7 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
     c->d_D3P = cv.take((size_t)3 * Np * npad * rs);
     c->d_LTP = cv.take((size_t)NF * npad * rs);
     c->d_D3Q = cv.take(std::max<size_t>(16, c->kt ? c->kt->pipe_blob_bytes : 0));
-    c->d_LTQ = nullptr;
+    c->d_LTQ = cv.take(std::max<size_t>(16, c->kt ? c->kt->tc_blob_bytes : 0));      // tensor-core kernel's tables
   }
   c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks);
   c->d_pt_src = (int*)cv.take((size_t)md.nslots * 4);

@@ -124,6 +124,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.ops = c->ops; a.ops.D3T = c->d_D3P; a.ops.LIFTT = c->d_LTP;
   a.ops2_D3Q = c->d_D3Q; a.ops2_LTQ = c->d_LTQ;
   const bool pipe = c->use_pipe && c->kt->pipe != nullptr;
+  const bool tc = c->use_tc && c->kt->tc != nullptr && o.nfields == 1;
   a.image = c->image; a.img_scratch = c->scratch; a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
   for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
   for (int fi = 0; fi < o.nfields; ++fi) {
@@ -180,7 +181,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     a.nblk = (int)md.nblocks - a.blk0;
     if (a.nblk > 0) {
       if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, pipe ? c->kt->pipe2(a, c->stream) : c->kt->step2(a, c->stream));
-      else DG_LAUNCH(c, KC_STEP, pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream));
+      else DG_LAUNCH(c, KC_STEP, tc ? c->kt->tc(a, c->stream) : (pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream)));
     }
     for (int l = lmin; l < L; ++l)
       for (int fi = 0; fi < o.nfields; ++fi) o.fields[fi]->par[l] ^= 1;

@@ -125,6 +125,7 @@ struct dg_ctx {
   char* d_D3Q = nullptr;                    // pipelined kernel's tile-packed tables
   char* d_LTQ = nullptr;
   bool use_pipe = true;                     // DGRTM_KERNEL=step selects the non-pipelined fused kernel
+  bool use_tc = false;                      // DGRTM_KERNEL=tc selects the tensor-core kernel (fp32, one wavefield)
   unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
   int* d_coarse[dgrtm::kMaxLevels];         // per level: slots with a finer face neighbour

@@ -159,7 +159,11 @@ struct KernelTable {
   void (*pipe2)(const StepArgs&, cudaStream_t);
   int pipe_TO, pipe_NT, pipe_RL, pipe_LL;
   size_t pipe_blob_bytes;
-  int (*pipe_set_const)(const void* blob_host, cudaStream_t);   // operator part of the blob -> constant memory                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
+  int (*pipe_set_const)(const void* blob_host, cudaStream_t);
+  // tensor-core variant (tc_kernel.cuh; fp32, one wavefield); tc == nullptr if not instantiated
+  void (*tc)(const StepArgs&, cudaStream_t);
+  int tc_K1, tc_K2, tc_NN;
+  size_t tc_blob_bytes;                                // [B1 hi | B1 lo | B2 hi | B2 lo | Fmask | perm table]   // operator part of the blob -> constant memory                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
   int (*init)();           // sets shared-memory attributes; returns cudaError
 };
 

@@ -1,5 +1,5 @@
 // One translation unit per order: compiled six times with -DDG_ORDER=1..6 (float and double each).
-#include "pipe_kernel.cuh"
+#include "tc_kernel.cuh"
 
 #ifndef DG_ORDER
 #error "compile with -DDG_ORDER=<1..6>"
@@ -64,6 +64,10 @@ template <typename real> struct Launch {
       e = cudaFuncSetAttribute(k_pipe<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PipeSmem<real, N>::bytes);
       if (e != cudaSuccess) return (int)e;
     }
+    if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled) {
+      e = cudaFuncSetAttribute(k_tc<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcSmem<N>::bytes);
+      if (e != cudaSuccess) return (int)e;
+    }
     const int th = 32 * Tiling<N>::T;
     occ_rhs = blocks_per_sm(k_rhs<real, N>, th, RhsSmem<real, N>::bytes);
     occ_upd = blocks_per_sm(k_update<real, N, 0>, th, UpdSmem<N>::template bytes<real>(1));
@@ -112,6 +116,12 @@ template <typename real> struct Launch {
     using C = PipeCfg<real, N>;
     launch_pdl(k_pipe<real, N, true>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
+  static void tc(const StepArgs& a, cudaStream_t s) {
+    if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled) {
+      if (a.nblk <= 0) return;
+      launch_pdl(k_tc<N>, a.nblk < kSMs ? a.nblk : kSMs, TcCfg<N>::G * 128, TcSmem<N>::bytes, s, a);
+    }
+  }
   static int pipe_set_const(const void* blob_host, cudaStream_t s) {
     if constexpr (PipeCfg<real, N>::enabled) {
       const size_t n = PipeSmem<real, N>::ops_reals * sizeof(real);
@@ -149,6 +159,11 @@ template <typename real> KernelTable make_table(int precision) {
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
   t.capture = Launch<real>::capture; t.init = Launch<real>::init;
   t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0; t.pipe_set_const = nullptr;
+  t.tc = nullptr; t.tc_K1 = t.tc_K2 = t.tc_NN = 0; t.tc_blob_bytes = 0;
+  if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled && TcSmem<N>::fits) {
+    t.tc = Launch<real>::tc; t.tc_K1 = TcSmem<N>::K1; t.tc_K2 = TcSmem<N>::K2; t.tc_NN = TcSmem<N>::NN;
+    t.tc_blob_bytes = TcSmem<N>::ops_bytes;
+  }
   if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
     t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
     t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;
