@@ -297,6 +297,9 @@ __global__ void __launch_bounds__(TcCfg<N>::G * 128, 1) k_tc(const __grid_consta
         tc_mma(tC, tbase + ks * 8, dB1h + off, IDESC, ks > 0);
         tc_mma(tC, tbase + KA + ks * 8, dB1h + off, IDESC, 1);
         tc_mma(tC, tbase + ks * 8, dB1l + off, IDESC, 1);
+#ifdef DG_TC_4TERM
+        tc_mma(tC, tbase + KA + ks * 8, dB1l + off, IDESC, 1);
+#endif
       }
       asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&full[2])) : "memory");
     }
@@ -349,6 +352,9 @@ __global__ void __launch_bounds__(TcCfg<N>::G * 128, 1) k_tc(const __grid_consta
         tc_mma(tC, tbase + ks * 8, dB2h + off, IDESC, 1);
         tc_mma(tC, tbase + KA + ks * 8, dB2h + off, IDESC, 1);
         tc_mma(tC, tbase + ks * 8, dB2l + off, IDESC, 1);
+#ifdef DG_TC_4TERM
+        tc_mma(tC, tbase + KA + ks * 8, dB2l + off, IDESC, 1);
+#endif
       }
       asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&full[2])) : "memory");
     }
