@@ -46,7 +46,10 @@ enum {
 enum { DG_BC_FREE = 1, DG_BC_ABSORBING = 2, DG_BC_RIGID = 3, DG_BC_PRESCRIBED = 4 };
 enum { DG_INTEGRATOR_AB3 = 0, DG_INTEGRATOR_LSERK4 = 1 };
 enum { DG_WAVELET_RICKER = 0 };
-enum { DG_IMAGING_CLASSICAL = 0, DG_IMAGING_CHARACTERISTIC = 1 };
+/* imaging condition (bit 0: characteristic variables (7) instead of p_S p_R (4)) and time quadrature (bit 1: the
+ * trapezoid rule (21) PAPER.md:178-180 instead of the Adams-Bashforth-consistent integral (22)-(24)) */
+enum { DG_IMAGING_CLASSICAL = 0, DG_IMAGING_CHARACTERISTIC = 1, DG_IMAGING_CLASSICAL_TRAPEZOID = 2,
+       DG_IMAGING_CHARACTERISTIC_TRAPEZOID = 3 };
 enum { DG_RHS_VOLUME = 0, DG_RHS_SURFACE = 1, DG_RHS_TOTAL = 2 };
 
 const char* dg_version(void);

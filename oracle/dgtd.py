@@ -405,7 +405,8 @@ class DGOracle:
     def accumulate_image(self, image, FS, FR, el, dts):
         order = int(FS.nhist[el[0]])
         co = ab_coefficients(order)
-        if image["mode"] == "characteristic":
+        trapezoid = image["mode"].endswith("_trapezoid")
+        if image["mode"].startswith("characteristic"):
             e = np.asarray(image["updir"], dtype=np.float64)
             Z = self.Z[el][:, None]
 
@@ -427,6 +428,12 @@ class DGOracle:
             acc = acc + dts * co["abar"][s] * (A * rB[s] + B * rA[s])
             for s2 in range(3):
                 acc = acc + dts * dts * co["C"][s, s2] * rA[s] * rB[s2]
+        if trapezoid:
+            # trapezoid rule (21) PAPER.md:178-180 (its printed "-" is a "+", reading Q1(v)): mean of the integrand at
+            # the two ends of the local step; the values at the new time are the update (18) of the combinations
+            A_new = A + dts * (co["a"][0] * rA[0] + co["a"][1] * rA[1] + co["a"][2] * rA[2])
+            B_new = B + dts * (co["a"][0] * rB[0] + co["a"][1] * rB[1] + co["a"][2] * rB[2])
+            acc = 0.5 * (A * B + A_new * B_new)
         image["I"][el] += abs(dts) * acc
 
     # -------------------------------------------------------------------------------------------

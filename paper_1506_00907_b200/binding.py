@@ -24,6 +24,7 @@ DG_BC_FREE, DG_BC_ABSORBING, DG_BC_RIGID, DG_BC_PRESCRIBED = 1, 2, 3, 4
 DG_INTEGRATOR_AB3, DG_INTEGRATOR_LSERK4 = 0, 1
 DG_WAVELET_RICKER = 0
 DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
+DG_IMAGING_CLASSICAL_TRAPEZOID, DG_IMAGING_CHARACTERISTIC_TRAPEZOID = 2, 3
 DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
 KERNEL_CLASSES = ("rhs", "update", "half", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
 

@@ -205,7 +205,7 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
   if (!ctx->have_final) throw ApiError(DG_ERR_STATE, "rtm_forward_shot first");
   if (nsteps < 1 || nsteps > ctx->final_nsteps) throw ApiError(DG_ERR_ARG, "nsteps must be in 1..(steps of the forward shot)");
   if (!updir) throw ApiError(DG_ERR_ARG, "updir is NULL");
-  if (imaging != DG_IMAGING_CLASSICAL && imaging != DG_IMAGING_CHARACTERISTIC) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
+  if (imaging < 0 || imaging > 3) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
   const int64_t ntot = ctx->final_nsteps;
   if (data) copy_data(ctx, nullptr, data, ntot * ctx->nlocal + 1);   // NULL: the signals recorded on the device
   // source field: restart from q(t_f) (history restarts, reading Q7); receiver field: from rest

@@ -125,7 +125,8 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.ops2_D3Q = c->d_D3Q; a.ops2_LTQ = c->d_LTQ;
   const bool pipe = c->use_pipe && c->kt->pipe != nullptr;
   const bool tc = c->use_tc && c->kt->tc != nullptr && o.nfields == 1;
-  a.image = c->image; a.img_scratch = c->scratch; a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
+  a.image = c->image; a.img_scratch = c->scratch; a.characteristic = (o.imaging & 1) != 0;
+  a.trapezoid = (o.imaging & 2) != 0;
   for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
   for (int fi = 0; fi < o.nfields; ++fi) {
     a.q[fi] = o.fields[fi]->q;

@@ -133,6 +133,7 @@ struct StepArgs {
   // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale
   const int* pt_index[2]; const void* pt_val[2]; double pt_scale[2];
   void* image; double e[3]; int characteristic;
+  int trapezoid;             // image integral by the trapezoid rule (21) instead of the AB-consistent (24)
   void* img_scratch;         // [block][4Np][32] scratch for the imaging scalars when they do not fit in shared memory
   OpsDev ops;                // D3T / LIFTT here are the PADDED tables: D3P [m][3][NPAD], LTP [j][NPAD]
   const void* ops2_D3Q;      // pipelined kernel: tile-packed tables D3Q [tile][m][RL], LTQ [tile][j][LL]

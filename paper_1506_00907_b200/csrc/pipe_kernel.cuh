@@ -571,6 +571,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
                 for (int k2 = 0; k2 < 3; ++k2) acc += dts * dts * (real)L.C[3 * k + k2] * rA[k] * rB[k2];
               }
+              if (a.trapezoid)                  // (21): mean of the integrand at the step ends; the new values are q + sum_s c_s r_s
+                acc = (real)0.5 * (S0 * A0 + (S0 + (c0 * rA[0] + c1 * rA[1] + c2 * rA[2])) * (A0 + (c0 * rB[0] + c1 * rB[1] + c2 * rB[2])));
               imgp[nn * 32] += adts * acc;
             }
           }

@@ -277,6 +277,26 @@ def test_rtm_shot_other_orders(precision, N, nlevels):
     g.close()
 
 
+@pytest.mark.parametrize("imaging,mode", [(2, "classical_trapezoid"), (3, "characteristic_trapezoid")])
+@pytest.mark.parametrize("precision,N", [(64, 3), (32, 3), (32, 4), (64, 2)])
+def test_rtm_trapezoid_imaging(precision, N, imaging, mode):
+    """Imaging with the trapezoid rule (21) instead of the AB-consistent integral (24): SURVEY.md 8(f) item 1."""
+    nsteps = 16
+    cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=N, nsteps=nsteps, n_receivers_side=3)
+    cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
+    o = make_oracle(cfg)
+    g = make_gpu(cfg, precision, history_steps=nsteps)
+    g.rtm_forward_shot(nsteps)
+    data_o, hist, qT = o.rtm_forward(nsteps)
+    g.rtm_backward_shot(nsteps, data_o, updir=cfg["updir"], imaging=imaging)
+    I_o, _, _ = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], mode=mode, nglobal_total=nsteps)
+    I_24, _, _ = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], mode=mode.replace("_trapezoid", ""),
+                                nglobal_total=nsteps)
+    assert np.abs(I_o).max() > 0 and rel_l2(I_o, I_24) > 1e-6          # the two quadratures really differ
+    assert rel_l2(g.rtm_image_read(), I_o) < (1e-4 if precision == 32 else 1e-10)
+    g.close()
+
+
 def test_rtm_first_image_step():
     cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=2, nsteps=40, n_receivers_side=3)
     cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)

@@ -377,3 +377,30 @@ def test_trace_history_layout_multirate():
     for l in range(3):
         sel = hist.faces[l]
         assert np.array_equal(hist.records[l][-1], qf[dg.bnd_k[sel], dg.bnd_f[sel]])
+
+
+def test_trapezoid_image_rule_closed_form():
+    """(21) on fields linear in time over one step: integrand f(t) = (A + t rA)(B + t rB) is a quadratic, the
+    trapezoid rule overshoots its integral by exactly rA rB dt^3 / 6, the AB-consistent rule (24) is exact."""
+    from oracle.dgtd import DGOracle
+    from workloads import box_tet_mesh
+    etov, vx = box_tet_mesh(1, 1, 1)
+    dg = DGOracle(2, etov, vx, default_bc=2)
+    dg.set_model(np.ones(dg.K), np.ones(dg.K), 1, 0.15)
+    rng = np.random.default_rng(5)
+    FS, FR = dg.new_field(rng.standard_normal((dg.K, 4, dg.Np))), dg.new_field(rng.standard_normal((dg.K, 4, dg.Np)))
+    rS, rR = rng.standard_normal((dg.K, 4, dg.Np)), rng.standard_normal((dg.K, 4, dg.Np))
+    for F, r in ((FS, rS), (FR, rR)):
+        F.hist[:] = r[None]                      # constant right-hand side: the field is linear in time
+        F.nhist[:] = 3
+    el = np.arange(dg.K)
+    dt = 0.37
+    A, B, rA, rB = FS.q[:, 0], FR.q[:, 0], rS[:, 0], rR[:, 0]
+    exact = dt * A * B + dt ** 2 / 2 * (A * rB + B * rA) + dt ** 3 / 3 * rA * rB
+    out = {}
+    for mode in ("classical", "classical_trapezoid"):
+        image = dict(I=np.zeros((dg.K, dg.Np)), mode=mode, updir=(0.0, 0.0, -1.0))
+        dg.accumulate_image(image, FS, FR, el, dt)
+        out[mode] = image["I"]
+    assert np.abs(out["classical"] - exact).max() < 1e-12 * np.abs(exact).max()
+    assert np.abs(out["classical_trapezoid"] - (exact + dt ** 3 / 6 * rA * rB)).max() < 1e-12 * np.abs(exact).max()
