@@ -82,7 +82,8 @@ int dg_set_dt(dg_ctx* ctx, double dt_local);
  * scaling of eq (1): reading Q5; owner element: reading Q11).  Ricker f(t) = amp (1-2a) exp(-a),
  * a = (pi f0 (t-tp))^2. */
 int dg_set_source(dg_ctx* ctx, const double x0[3], int wavelet, double f0, double tp, double amp);
-/* nr receivers xr[nr][3]: sampling rows l_n(x_r) and injection weights M_k^-1 l(x_r) (eq (15)). */
+/* nr receivers xr[nr][3]: sampling rows l_n(x_r) and injection weights M_k^-1 l(x_r) (eq (15)).  The RTM region is
+ * sized by nr: a new receiver set unbinds it (read the image first, then rtm_history_bytes / rtm_bind_history again). */
 int dg_set_receivers(dg_ctx* ctx, int64_t nr, const double* xr);
 
 /* Device memory.  The library allocates none: query, allocate (e.g. a torch tensor), bind.

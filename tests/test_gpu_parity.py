@@ -297,6 +297,40 @@ def test_rtm_trapezoid_imaging(precision, N, imaging, mode):
     g.close()
 
 
+def test_two_shot_survey_stacks_images():
+    """several gathers over one mesh: the set-up (operators, geometry,
+    connectivity, levels) is reused, source and receivers change between shots, the images add up."""
+    nsteps = 24
+    cfg = make_config("cfg4_rtm", hexes=(5, 4, 3), N=3, nsteps=nsteps, n_receivers_side=3)
+    shots = [dict(x0=cfg["source"]["x0"], rcv=cfg["receivers"]),
+             dict(x0=cfg["source"]["x0"] + np.array([0.41, -0.33, 0.05]), rcv=cfg["receivers"][::2] + np.array([0.07, 0.03, 0.0]))]
+    g = make_gpu(cfg, 64)
+    I_sum = 0.0
+    for sh in shots:
+        c2 = dict(cfg, source=dict(cfg["source"], x0=sh["x0"], f0=60.0, tp=0.01), receivers=sh["rcv"])
+        o = make_oracle(c2)
+        data_o, hist, qT = o.rtm_forward(nsteps)
+        I_o, _, _ = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], nglobal_total=nsteps)
+        I_sum = I_sum + I_o
+        # the RTM region is sized by the receiver count: a new receiver set needs a new region, so the image so far is
+        # read out first and the stack continues on the host (same receiver set: no re-bind, the image stacks in place)
+        img = g.rtm_image_read() if g._hist is not None else None
+        g.dg_set_source(sh["x0"], 60.0, 0.01, 1.0)
+        g.dg_set_receivers(sh["rcv"])
+        g.bind_history_torch(nsteps)
+        if img is not None:
+            assert np.abs(g.rtm_image_read()).max() == 0                  # a fresh history region starts from zero
+        data_g = g.rtm_forward_shot(nsteps)
+        assert rel_l2(data_g, data_o) < 1e-10
+        g.rtm_backward_shot(nsteps, data_o, updir=cfg["updir"])
+        if img is not None:
+            I_g = img + g.rtm_image_read()
+        else:
+            I_g = g.rtm_image_read()
+    assert rel_l2(I_g, I_sum) < 1e-10
+    g.close()
+
+
 def test_rtm_first_image_step():
     cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=2, nsteps=40, n_receivers_side=3)
     cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
