@@ -27,7 +27,10 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #define DG_P3_G 3
 #define DG_P3_RS 1
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = 2, RS = DG_P3_RS, UG = 0; };
+#ifndef DG_P3_QS
+#define DG_P3_QS 2
+#endif
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = 0; };
 #ifndef DG_P4_TO
 #define DG_P4_TO 7
 #define DG_P4_NT 5
