@@ -302,9 +302,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
       if (f < 4 && c >= 0) {
         const int s2 = c >> 2;
         const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC;
-        real* dst = TR + ((size_t)f * 32 + lane) * REC;
+        real* dst = TR + ((size_t)f * (REC / CPW) * 32 + lane) * CPW;   // [face][piece][lane][CPW]: a warp's pieces are contiguous
 #pragma unroll
-        for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * CPW, src + v * CPW);
+        for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * 32 * CPW, src + v * CPW);
       }
     }
   };
@@ -366,11 +366,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
           real ep[Nfp], ev[Nfp];
           {
             real rv[REC];
-            const real* src = TR + ((size_t)f * 32 + lane) * REC;
+            const real* src = TR + ((size_t)f * (REC / CPW) * 32 + lane) * CPW;
             using V = typename VecT<real, CPW>::T;
 #pragma unroll
             for (int v = 0; v < REC / CPW; ++v) {
-              const V x = reinterpret_cast<const V*>(src)[v];
+              const V x = reinterpret_cast<const V*>(src)[v * 32];
               const real* xs = reinterpret_cast<const real*>(&x);
 #pragma unroll
               for (int e = 0; e < CPW; ++e) rv[v * CPW + e] = xs[e];

@@ -155,9 +155,9 @@ __global__ void __launch_bounds__(TcCfg<N>::G * 128, 1) k_tc(const __grid_consta
       const int s2 = code >> 2;
       const real* qf = static_cast<const real*>(s2 >= slot_hi ? a.lv[lp].qf_read[0] : (s2 < slot_lo ? a.lv[lm].qf_read[0] : L.qf_read[0]));
       const real* src = qf + (size_t)code * REC;
-      real* dst = TR + ((size_t)w * 32 + lane) * REC;
+      real* dst = TR + ((size_t)w * (REC / CPW) * 32 + lane) * CPW;     // [face][piece][lane][CPW]: a warp's pieces are contiguous
 #pragma unroll
-      for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * CPW, src + v * CPW);
+      for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * 32 * CPW, src + v * CPW);
     }
   };
 
@@ -200,11 +200,11 @@ __global__ void __launch_bounds__(TcCfg<N>::G * 128, 1) k_tc(const __grid_consta
       real ep[Nfp], ev[Nfp];
       {
         real rv[REC];
-        const real* src = TR + ((size_t)f * 32 + lane) * REC;
+        const real* src = TR + ((size_t)f * (REC / CPW) * 32 + lane) * CPW;
         using V = typename VecT<real, CPW>::T;
 #pragma unroll
         for (int v = 0; v < REC / CPW; ++v) {
-          const V x = reinterpret_cast<const V*>(src)[v];
+          const V x = reinterpret_cast<const V*>(src)[v * 32];
           const real* xs = reinterpret_cast<const real*>(&x);
 #pragma unroll
           for (int e = 0; e < CPW; ++e) rv[v * CPW + e] = xs[e];
