@@ -296,15 +296,24 @@ k_pipe(const __grid_constant__ StepArgs a) {
     const real* qfm = static_cast<const real*>(a.lv[lm].qf_read[fi]);
     const real* qf0 = static_cast<const real*>(L.qf_read[fi]);
     const real* qfp = static_cast<const real*>(a.lv[lp].qf_read[fi]);
+    // cooperative gather: consecutive lanes fetch consecutive 16-byte pieces of the SAME neighbour record (a
+    // record is one contiguous line or two), so an instruction touches ~NP times fewer lines than one record per
+    // lane would; piece P = it*32 + lane belongs to element-lane r = P / NP, whose code comes by shuffle
+    constexpr int NP = REC / CPW;
 #pragma unroll
     for (int k = 0; k < FPW; ++k) {
-      const int f = w + k * NT, c = code[k];
-      if (f < 4 && c >= 0) {
-        const int s2 = c >> 2;
-        const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC;
-        real* dst = TR + ((size_t)f * (REC / CPW) * 32 + lane) * CPW;   // [face][piece][lane][CPW]: a warp's pieces are contiguous
+      const int f = w + k * NT;
+      if (f < 4) {
 #pragma unroll
-        for (int v = 0; v < REC / CPW; ++v) cp_async<CPB>(dst + v * 32 * CPW, src + v * CPW);
+        for (int it = 0; it < NP; ++it) {
+          const int P = it * 32 + lane, r = P / NP, v = P - r * NP;
+          const int c = __shfl_sync(0xffffffffu, code[k], r);
+          if (c >= 0) {
+            const int s2 = c >> 2;
+            const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC + v * CPW;
+            cp_async<CPB>(TR + ((size_t)f * 32 + r) * REC + v * CPW, src);      // [face][element-lane][REC]: a warp writes 512 contiguous bytes
+          }
+        }
       }
     }
   };
@@ -339,6 +348,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     if (QS == 1 && i > 0) issue_q(i, 0);
     mbar_wait(&full[s], (unsigned)(QS == 2 ? (i >> 1) : i) & 1u);
     cp_async_wait_all();
+    __syncwarp();                               // the pieces of my record were fetched by other lanes of this warp
     const real rc2 = geo[GEO_RC2 * 32], irho = geo[GEO_IRHO * 32];
     real vold[3][TO];                                             // this tile's velocities before the in-place transform
     if (INPLACE) {
@@ -366,11 +376,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
           real ep[Nfp], ev[Nfp];
           {
             real rv[REC];
-            const real* src = TR + ((size_t)f * (REC / CPW) * 32 + lane) * CPW;
+            const real* src = TR + ((size_t)f * 32 + lane) * REC;
             using V = typename VecT<real, CPW>::T;
 #pragma unroll
             for (int v = 0; v < REC / CPW; ++v) {
-              const V x = reinterpret_cast<const V*>(src)[v * 32];
+              const V x = reinterpret_cast<const V*>(src)[v];
               const real* xs = reinterpret_cast<const real*>(&x);
 #pragma unroll
               for (int e = 0; e < CPW; ++e) rv[v * CPW + e] = xs[e];
