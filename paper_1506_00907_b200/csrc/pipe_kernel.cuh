@@ -622,26 +622,31 @@ k_pipe(const __grid_constant__ StepArgs a) {
         if (f < 4) {
           const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
           const int* prow = sP + ((wp >> (8 * f)) & 255) * Nfp;
-          real* st = pen + f * REC * 32 + lane;
+          // staging [row][lane] with the lane rotated by row / VS: conflict-free for these stores (rows of one
+          // instruction lie within one face) and for the piece-wise reads of the write-out below
+          constexpr int VS = 16 / (int)sizeof(real);
 #pragma unroll
           for (int i2 = 0; i2 < Nfp; ++i2) {
             const int o = fofs[k][i2], pos = prow[i2];
-            st[pos * 32] = Q[o];
-            st[(Nfp + pos) * 32] = nx * Q[Np * 32 + o] + ny * Q[2 * Np * 32 + o] + nz * Q[3 * Np * 32 + o];
+            const int rp = f * REC + pos, rv = rp + Nfp;
+            pen[rp * 32 + ((lane + rp / VS) & 31)] = Q[o];
+            pen[rv * 32 + ((lane + rv / VS) & 31)] = nx * Q[Np * 32 + o] + ny * Q[2 * Np * 32 + o] + nz * Q[3 * Np * 32 + o];
           }
         }
       }
       group_sync<NT>(g);
-      {
+      {  // cooperative write-out: the block's 32 x 4 records are one contiguous run; consecutive lanes store
+         // consecutive 16-byte pieces (piece P = element-lane P / NV, rows VS (P % NV) ..)
         constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
         using V = typename VecT<real, VS>::T;
-        real* dst = static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + ((size_t)b * 32 + lane) * ROWS;
-        for (int v = w; v < NV; v += NT) {
+        V* dst = reinterpret_cast<V*>(static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + (size_t)b * 32 * ROWS);
+        for (int it = w; it < NV; it += NT) {
+          const int P = it * 32 + lane, el = P / NV, o4 = P - el * NV;
           V x;
           real* xs = reinterpret_cast<real*>(&x);
 #pragma unroll
-          for (int e = 0; e < VS; ++e) xs[e] = pen[(v * VS + e) * 32 + lane];
-          reinterpret_cast<V*>(dst)[v] = x;
+          for (int e = 0; e < VS; ++e) xs[e] = pen[(o4 * VS + e) * 32 + ((el + o4) & 31)];
+          dst[P] = x;
         }
       }
     }
