@@ -23,14 +23,23 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 // (9 more FMAs per input node and warp, two shared-memory passes and one barrier fewer)
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
+#endif
+#ifndef DG_P3_NT
 #define DG_P3_NT 4
+#endif
+#ifndef DG_P3_G
 #define DG_P3_G 3
+#endif
+#ifndef DG_P3_RS
 #define DG_P3_RS 1
 #endif
 #ifndef DG_P3_QS
 #define DG_P3_QS 2
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = 0; };
+#ifndef DG_P3_UG
+#define DG_P3_UG 0
+#endif
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG; };
 #ifndef DG_P4_TO
 #define DG_P4_TO 7
 #define DG_P4_NT 5

@@ -437,24 +437,29 @@ k_step(const __grid_constant__ StepArgs a) {
                 const int pos = sP[((wp >> (8 * f)) & 255) * Nfp + i];
                 const real fnx = geo[(GEO_FACE + 5 * f + 0) * 32], fny = geo[(GEO_FACE + 5 * f + 1) * 32],
                            fnz = geo[(GEO_FACE + 5 * f + 2) * 32];
-                pen[(f * REC + pos) * 32 + lane] = rp[nn];
-                pen[(f * REC + Nfp + pos) * 32 + lane] = fnx * rx[nn] + fny * ry[nn] + fnz * rz[nn];
+                // staging [row][lane] with the lane rotated by row / VS (conflict-free piece-wise reads below)
+                constexpr int VSt = 16 / (int)sizeof(real);
+                const int rwp = f * REC + pos, rwv = rwp + Nfp;
+                pen[rwp * 32 + ((lane + rwp / VSt) & 31)] = rp[nn];
+                pen[rwv * 32 + ((lane + rwv / VSt) & 31)] = fnx * rx[nn] + fny * ry[nn] + fnz * rz[nn];
               }
             }
           }
         }
         group_sync<NT>(g);
-        // each lane writes its own element's 4 records (8Nfp contiguous reals), VS reals per store
+        // cooperative write-out: the block's 32 x 4 records are one contiguous run; consecutive lanes store
+        // consecutive 16-byte pieces (piece P = element-lane P / NV, rows VS (P % NV) ..)
         {
           constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
           using V = typename VecT<real, VS>::T;
-          real* dst = static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + ((size_t)b * 32 + lane) * ROWS;
-          for (int v = w; v < NV; v += NT) {
+          V* dst = reinterpret_cast<V*>(static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + (size_t)b * 32 * ROWS);
+          for (int it = w; it < NV; it += NT) {
+            const int P = it * 32 + lane, el = P / NV, o4 = P - el * NV;
             V x;
             real* xs = reinterpret_cast<real*>(&x);
 #pragma unroll
-            for (int e = 0; e < VS; ++e) xs[e] = pen[(v * VS + e) * 32 + lane];
-            reinterpret_cast<V*>(dst)[v] = x;
+            for (int e = 0; e < VS; ++e) xs[e] = pen[(o4 * VS + e) * 32 + ((el + o4) & 31)];
+            dst[P] = x;
           }
         }
       }
