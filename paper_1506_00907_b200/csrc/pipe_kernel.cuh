@@ -454,6 +454,12 @@ k_pipe(const __grid_constant__ StepArgs a) {
     load_codes(i + 2, codeC);
     const int wp = a.wperm[(size_t)b * 32 + lane];
     const int pi = a.pt_index[fi] ? a.pt_index[fi][(size_t)b * 32 + lane] : -1;
+    real imgv[TO];                              // image values of this tile, fetched long before their update
+    if (DUAL && fi == 1 && L.image_on) {
+      const real* ip = static_cast<const real*>(a.image) + ((size_t)b * Np + n0) * 32 + lane;
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) imgv[nn] = (TO * NT == Np || n0 + nn < Np) ? ip[nn * 32] : (real)0;
+    }
     if (INPLACE) {                              // v -> (U.Gr, U.Gs, U.Gt) once per block (Alg. 2)
       for (int m = w; m < Np; m += NT) {
         const real vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
@@ -595,7 +601,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
               }
               if (a.trapezoid)                  // (21): mean of the integrand at the step ends; the new values are q + sum_s c_s r_s
                 acc = (real)0.5 * (S0 * A0 + (S0 + (c0 * rA[0] + c1 * rA[1] + c2 * rA[2])) * (A0 + (c0 * rB[0] + c1 * rB[1] + c2 * rB[2])));
-              imgp[nn * 32] += adts * acc;
+              imgp[nn * 32] = imgv[nn] + adts * acc;
             }
           }
           // value at the half step (19) = new value + sum_s d_s r_s; kept for the second trace pass
