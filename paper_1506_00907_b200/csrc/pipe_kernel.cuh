@@ -41,12 +41,21 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #endif
 template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG; };
 #ifndef DG_P4_TO
-#define DG_P4_TO 7
-#define DG_P4_NT 5
+#define DG_P4_TO 9
+#endif
+#ifndef DG_P4_NT
+#define DG_P4_NT 4
+#endif
+#ifndef DG_P4_G
 #define DG_P4_G 3
+#endif
+#ifndef DG_P4_RS
 #define DG_P4_RS 0
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = 1; };
+#ifndef DG_P4_UG
+#define DG_P4_UG 1
+#endif
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = DG_P4_UG; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
