@@ -467,7 +467,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, N, precision); None until captured
-NCU_TRAFFIC = {("cfg2_two_layer", 3, 32): 196859904}      # profiles/r1b_fused_pipeline.md (147.65 MB read + 49.21 MB written)
+NCU_TRAFFIC = {("cfg2_two_layer", 3, 32): 199077632}      # profiles/r1b_fused_pipeline.md (148.27 MB read + 50.81 MB written)
 
 
 if __name__ == "__main__":

@@ -369,13 +369,13 @@ def test_cfg5_orders(N, precision):
 # full BASELINE.json sizes in the launch configuration bench.py times (every CTA, every group of the
 # pipelined kernel, ragged chunks): a few steps from a random state, every element compared
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name,nsteps", [("cfg2_two_layer", 5), ("cfg4_rtm", 2)])
+@pytest.mark.parametrize("name,nsteps", [("cfg2_two_layer", 5), ("cfg4_rtm", 2), ("cfg3_lts", 1)])
 def test_full_size_short_run(name, nsteps):
     cfg = make_config(name)
     cfg["receivers"] = None
     o = make_oracle(cfg)
     g = make_gpu(cfg, 32)
-    assert g.K == {"cfg2_two_layer": 98304, "cfg4_rtm": 786432}[name]
+    assert g.K == {"cfg2_two_layer": 98304, "cfg4_rtm": 786432, "cfg3_lts": 331776}[name]
     q0 = random_state(o.K, o.Np, 11)
     g.dg_set_state(q0)
     g.dg_step(nsteps)
