@@ -305,6 +305,10 @@ k_pipe(const __grid_constant__ StepArgs a) {
       bulk_prefetch_l2(static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES);
     }
   };
+  // piece P = it*32 + lane of a face's 32 records belongs to element-lane P / NP, offset (P % NP) CPW in its record
+  int gth_r[REC / CPW], gth_v[REC / CPW];
+#pragma unroll
+  for (int it = 0; it < REC / CPW; ++it) { const int P = it * 32 + lane; gth_r[it] = P / (REC / CPW); gth_v[it] = (P - gth_r[it] * (REC / CPW)) * CPW; }
   // the neighbours' trace records of item i (per-lane cp.async by their consumer lanes)
   auto issue_tr = [&](int i, const int (&code)[FPW]) {
     const int b = item_block(i), fi = i % NFLD, l = level_of(b);
@@ -324,12 +328,12 @@ k_pipe(const __grid_constant__ StepArgs a) {
       if (f < 4) {
 #pragma unroll
         for (int it = 0; it < NP; ++it) {
-          const int P = it * 32 + lane, r = P / NP, v = P - r * NP;
-          const int c = __shfl_sync(0xffffffffu, code[k], r);
+          const int c = __shfl_sync(0xffffffffu, code[k], gth_r[it]);
           if (c >= 0) {
             const int s2 = c >> 2;
-            const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC + v * CPW;
-            cp_async<CPB>(TR + ((size_t)f * 32 + r) * REC + v * CPW, src);      // [face][element-lane][REC]: a warp writes 512 contiguous bytes
+            const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC + gth_v[it];
+            // [face][element-lane][REC] = [face][piece P]: a warp writes 512 contiguous bytes
+            cp_async<CPB>(TR + (size_t)f * 32 * REC + (it * 32 + lane) * CPW, src);
           }
         }
       }
