@@ -305,6 +305,15 @@ k_pipe(const __grid_constant__ StepArgs a) {
       bulk_prefetch_l2(static_cast<const real*>(a.geo) + (size_t)b * DG_NGEO * 32, GBYTES);
     }
   };
+  // write-out pieces of this warp (it = w + k NT): staging offset of piece P = it*32 + lane (rows VS (P % NV) .. of
+  // element-lane P / NV, column rotated by the piece index)
+  constexpr int WO_VS = 16 / (int)sizeof(real), WO_NV = 4 * REC / WO_VS, WOK = (WO_NV + NT - 1) / NT;
+  int wo_src[WOK];
+#pragma unroll
+  for (int k = 0; k < WOK; ++k) {
+    const int P = (w + k * NT) * 32 + lane, el = P / WO_NV, o4 = P - el * WO_NV;
+    wo_src[k] = o4 * WO_VS * 32 + ((el + o4) & 31);
+  }
   // piece P = it*32 + lane of a face's 32 records belongs to element-lane P / NP, offset (P % NP) CPW in its record
   int gth_r[REC / CPW], gth_v[REC / CPW];
 #pragma unroll
@@ -668,13 +677,16 @@ k_pipe(const __grid_constant__ StepArgs a) {
         constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
         using V = typename VecT<real, VS>::T;
         V* dst = reinterpret_cast<V*>(static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + (size_t)b * 32 * ROWS);
-        for (int it = w; it < NV; it += NT) {
-          const int P = it * 32 + lane, el = P / NV, o4 = P - el * NV;
-          V x;
-          real* xs = reinterpret_cast<real*>(&x);
 #pragma unroll
-          for (int e = 0; e < VS; ++e) xs[e] = pen[(o4 * VS + e) * 32 + ((el + o4) & 31)];
-          dst[P] = x;
+        for (int k = 0; k < WOK; ++k) {
+          const int it = w + k * NT;
+          if (it < NV) {
+            V x;
+            real* xs = reinterpret_cast<real*>(&x);
+#pragma unroll
+            for (int e = 0; e < VS; ++e) xs[e] = pen[wo_src[k] + e * 32];
+            dst[it * 32 + lane] = x;
+          }
         }
       }
     }
