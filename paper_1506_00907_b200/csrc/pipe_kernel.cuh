@@ -337,10 +337,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
       if (f < 4) {
 #pragma unroll
         for (int it = 0; it < NP; ++it) {
-          const int c = __shfl_sync(0xffffffffu, code[k], gth_r[it]);
+          const int gr = gth_r[it], gv = gth_v[it];
+          const int c = __shfl_sync(0xffffffffu, code[k], gr);
           if (c >= 0) {
             const int s2 = c >> 2;
-            const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC + gth_v[it];
+            const real* src = (s2 >= slot_hi ? qfp : (s2 < slot_lo ? qfm : qf0)) + (size_t)c * REC + gv;
             // [face][element-lane][REC] = [face][piece P]: a warp writes 512 contiguous bytes
             cp_async<CPB>(TR + (size_t)f * 32 * REC + (it * 32 + lane) * CPW, src);
           }
@@ -677,15 +678,26 @@ k_pipe(const __grid_constant__ StepArgs a) {
         constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
         using V = typename VecT<real, VS>::T;
         V* dst = reinterpret_cast<V*>(static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + (size_t)b * 32 * ROWS);
-#pragma unroll
-        for (int k = 0; k < WOK; ++k) {
-          const int it = w + k * NT;
-          if (it < NV) {
+        if constexpr (DUAL) {                   // register-bound: a rolled loop that recomputes the piece offsets
+          for (int it = w; it < NV; it += NT) {
+            const int P = it * 32 + lane, el = P / NV, o4 = P - el * NV;
             V x;
             real* xs = reinterpret_cast<real*>(&x);
 #pragma unroll
-            for (int e = 0; e < VS; ++e) xs[e] = pen[wo_src[k] + e * 32];
-            dst[it * 32 + lane] = x;
+            for (int e = 0; e < VS; ++e) xs[e] = pen[(o4 * VS + e) * 32 + ((el + o4) & 31)];
+            dst[P] = x;
+          }
+        } else {
+#pragma unroll
+          for (int k = 0; k < WOK; ++k) {
+            const int it = w + k * NT;
+            if (it < NV) {
+              V x;
+              real* xs = reinterpret_cast<real*>(&x);
+#pragma unroll
+              for (int e = 0; e < VS; ++e) xs[e] = pen[wo_src[k] + e * 32];
+              dst[it * 32 + lane] = x;
+            }
           }
         }
       }
