@@ -6,7 +6,7 @@ this package; the CUDA path shares no code with it.
 What is computed (PAPER.md = /root/reference/PAPER.md):
   * nodes: N_p = (N+1)(N+2)(N+3)/6 warp-and-blend nodes (PAPER.md:96, eq. (9)-(10) context;
     construction per Warburton 2006 as read in DESIGN.md reading Q10 - the exact nodes of the paper
-    are "parity unpinned", only their properties are pinned in tests/test_oracle_reference_element.py)
+    are "parity unpinned", only their properties are pinned in tests/test_oracle_operators.py)
   * D_j (differentiation matrices), M (mass), L_f (lifting matrices)  (App. A 593-612)
 
 Construction route (deliberately different from the CUDA library's host setup, which uses monomials
