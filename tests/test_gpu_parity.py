@@ -247,15 +247,16 @@ def test_cfg4_rtm_shot(precision, nlevels, imaging):
     g.close()
 
 
-@pytest.mark.parametrize("precision,N,nlevels", [(32, 4, 1), (32, 4, 3), (64, 3, 3), (32, 5, 1), (64, 4, 1), (32, 1, 3)])
+@pytest.mark.parametrize("precision,N,nlevels", [(32, 4, 1), (32, 4, 3), (64, 3, 3), (32, 5, 1), (64, 4, 1), (32, 1, 3),
+                                                 (64, 6, 1), (32, 6, 1), (64, 5, 3), (32, 2, 1)])
 def test_rtm_shot_other_orders(precision, N, nlevels):
     """The two-wavefield kernels of the other orders / precisions (several warps per element block, padded
     output tiles, imaging scalars in registers, shared or global memory): forward + backward + image."""
     nsteps = 16
     if nlevels == 1:
-        cfg = make_config("cfg4_rtm", hexes=(4, 4, 3), N=N, nsteps=nsteps, n_receivers_side=3)
+        cfg = make_config("cfg4_rtm", hexes=(4, 4, 3) if N < 6 else (3, 3, 2), N=N, nsteps=nsteps, n_receivers_side=3)
     else:
-        cfg = make_config("cfg3_lts", hexes=(5, 5, 6), N=N, nsteps=nsteps)
+        cfg = make_config("cfg3_lts", hexes=(5, 5, 6) if N < 5 else (4, 4, 5), N=N, nsteps=nsteps)
         gx = np.linspace(0.4, 2.6, 3)
         cfg["receivers"] = np.array([[x + 0.013, y + 0.007, 0.06] for x in gx for y in gx])
         cfg["updir"] = np.array([0.0, 0.0, -1.0])
