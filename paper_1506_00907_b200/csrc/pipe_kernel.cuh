@@ -18,9 +18,14 @@ namespace dgrtm {
 // ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
 // RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: read from global in the
 // update phase after an L2 prefetch (saves 8Np rows of shared memory per group: more groups per SM)
-template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1; };
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0; };
+// F2 = 1: the volume contraction of the one-field fp32 kernel uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the
+// FMA instructions for twice the accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 977 -> 1020 us)
 // UG = 1: velocities -> U.G once per block, in place in shared memory; 0: every warp forms U.G on the fly
 // (9 more FMAs per input node and warp, two shared-memory passes and one barrier fewer)
+#ifndef DG_PIPE_FFMA2
+#define DG_PIPE_FFMA2 1
+#endif
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #endif
@@ -39,7 +44,7 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #ifndef DG_P3_UG
 #define DG_P3_UG 0
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG; };
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG, F2 = DG_PIPE_FFMA2; };
 #ifndef DG_P4_TO
 #define DG_P4_TO 9
 #endif
@@ -55,14 +60,14 @@ template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; sta
 #ifndef DG_P4_UG
 #define DG_P4_UG 1
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = DG_P4_UG; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
 #define DG_D3_G 3
 #endif
 #ifndef DG_D3_OFF
-template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0; };
+template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0, F2 = 0; };
 #endif
 
 template <typename real, int N> struct PipeSmem {
@@ -501,6 +506,43 @@ k_pipe(const __grid_constant__ StepArgs a) {
       pipe_tile_dispatch<real, N, 0>(w, Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
     }
 #else
+    if constexpr (sizeof(real) == 4 && !DUAL && Cfg::F2) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
+                                                 // (the two-field kernel is register-bound and keeps scalar FMAs)
+      float2 aG2[RL / 2], aD2[RL / 2];
+#pragma unroll
+      for (int k = 0; k < RL / 2; ++k) { aG2[k] = make_float2(0.f, 0.f); aD2[k] = make_float2(0.f, 0.f); }
+      constexpr int UM2 = 5;
+#pragma unroll UM2
+      for (int m = 0; m < Np; ++m) {
+        const float p = Q[m * 32 + lane];
+        const float vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
+        float ur, us, ut;
+        if (INPLACE) { ur = vx; us = vy; ut = vz; }
+        else { ur = g00 * vx + g10 * vy + g20 * vz; us = g01 * vx + g11 * vy + g21 * vz; ut = g02 * vx + g12 * vy + g22 * vz; }
+        float d[RL];
+        load_packed<float, RL>(reinterpret_cast<const float*>(myD) + m * RL, d);
+        const float2 pp = make_float2(p, p);
+#pragma unroll
+        for (int k = 0; k < RL / 2; ++k) {
+          const int e0 = 2 * k, e1 = 2 * k + 1;
+          const float u0 = e0 < TO ? ur : (e0 < 2 * TO ? us : (e0 < 3 * TO ? ut : 0.f));
+          const float u1 = e1 < TO ? ur : (e1 < 2 * TO ? us : (e1 < 3 * TO ? ut : 0.f));
+          const float2 dk = make_float2(d[e0], d[e1]);
+          aG2[k] = __ffma2_rn(dk, pp, aG2[k]);
+          aD2[k] = __ffma2_rn(dk, make_float2(u0, u1), aD2[k]);
+        }
+      }
+      const float* fG = reinterpret_cast<const float*>(aG2);
+      const float* fD = reinterpret_cast<const float*>(aD2);
+#pragma unroll
+      for (int nn = 0; nn < TO; ++nn) {
+        const float aDn = fD[nn] + fD[TO + nn] + fD[2 * TO + nn], aRn = fG[nn], aSn = fG[TO + nn], aTn = fG[2 * TO + nn];
+        rp[nn] = -rc2 * aDn;
+        rx[nn] = -irho * (g00 * aRn + g01 * aSn + g02 * aTn);
+        ry[nn] = -irho * (g10 * aRn + g11 * aSn + g12 * aTn);
+        rz[nn] = -irho * (g20 * aRn + g21 * aSn + g22 * aTn);
+      }
+    } else
     {
       real aD[TO], aR[TO], aS[TO], aT[TO];
 #pragma unroll
