@@ -82,8 +82,10 @@ int dg_set_dt(dg_ctx* ctx, double dt_local);
  * scaling of eq (1): reading Q5; owner element: reading Q11).  Ricker f(t) = amp (1-2a) exp(-a),
  * a = (pi f0 (t-tp))^2. */
 int dg_set_source(dg_ctx* ctx, const double x0[3], int wavelet, double f0, double tp, double amp);
-/* nr receivers xr[nr][3]: sampling rows l_n(x_r) and injection weights M_k^-1 l(x_r) (eq (15)).  The RTM region is
- * sized by nr: a new receiver set unbinds it (read the image first, then rtm_history_bytes / rtm_bind_history again). */
+/* nr receivers xr[nr][3]: sampling rows l_n(x_r) and injection weights M_k^-1 l(x_r) (eq (15)).  The receiver-sized part
+ * of the RTM region holds max(nr at bind time, rtm_set_receiver_capacity) receivers: a new receiver set within that
+ * capacity keeps the region (image, q(t_f) and trace history untouched: the gathers of a survey stack in place,
+ * PAPER.md:61, 460, 478); a larger one unbinds it (rtm_history_bytes / rtm_bind_history again; the image restarts). */
 int dg_set_receivers(dg_ctx* ctx, int64_t nr, const double* xr);
 
 /* Device memory.  The library allocates none: query, allocate (e.g. a torch tensor), bind.
@@ -112,6 +114,7 @@ int dg_set_exterior(dg_ctx* ctx, const double* ext);
  * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side
  * evaluation time of its owner plus the final time (layout reading Q12) - it stays in
  * HBM.  rtm_history_bytes: size for shots of nsteps global steps. */
+int rtm_set_receiver_capacity(dg_ctx* ctx, int64_t max_receivers);   /* before rtm_history_bytes / rtm_bind_history */
 int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n);
 int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n);
 /* Forward phase: from rest at t = 0, source on, nsteps global steps; captures the boundary traces,
@@ -131,6 +134,11 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
                       int imaging, int64_t first_image_step);
 int rtm_image_read(dg_ctx* ctx, double* I_out /* [K][Np] */);
 int rtm_image_zero(dg_ctx* ctx);
+/* Device address and size of the image in the library's blocked layout [block][Np][32] (device precision), inside the
+ * caller's history buffer.  For the one collective of a shot-per-GPU survey: replicas
+ * that hold the same mesh and model share the layout, so their images add element-wise in place (e.g. one NCCL
+ * all-reduce over a view of the caller's buffer); rtm_image_read then returns the stacked image.  Synchronises. */
+int rtm_image_device(dg_ctx* ctx, void** dptr, size_t* nbytes);
 
 /* ---- getters (parity checks; all synchronise) ----------------------------------------------------*/
 int dg_get_sizes(const dg_ctx* ctx, int64_t* K, int* Np, int* Nfp, int64_t* nbnd, int64_t* nr);

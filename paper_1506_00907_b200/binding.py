@@ -26,7 +26,7 @@ DG_WAVELET_RICKER = 0
 DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
 DG_IMAGING_CLASSICAL_TRAPEZOID, DG_IMAGING_CHARACTERISTIC_TRAPEZOID = 2, 3
 DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
-KERNEL_CLASSES = ("rhs", "update", "half", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
+KERNEL_CLASSES = ("rhs", "update", "unused", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
 
 _vp, _i, _i64, _d, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_size_t
 _pd = C.POINTER(C.c_double)
@@ -52,12 +52,14 @@ SIGNATURES = {
     "dg_set_state": (_i, [_vp, _pd, _d]),
     "dg_step": (_i, [_vp, _i]),
     "dg_set_exterior": (_i, [_vp, _pd]),
+    "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
     "rtm_history_bytes": (_i, [_vp, _i, _psz]),
     "rtm_bind_history": (_i, [_vp, _vp, _sz]),
     "rtm_forward_shot": (_i, [_vp, _i, _pd]),
     "rtm_backward_shot": (_i, [_vp, _i, _pd, _pd, _i, _i64]),
     "rtm_image_read": (_i, [_vp, _pd]),
     "rtm_image_zero": (_i, [_vp]),
+    "rtm_image_device": (_i, [_vp, C.POINTER(_vp), _psz]),
     "dg_get_sizes": (_i, [_vp, _pi64, _pint, _pint, _pi64, _pi64]),
     "dg_get_nodes": (_i, [_vp, _pd, _pd, _pd]),
     "dg_get_operators": (_i, [_vp, _pd, _pd, _pd, _pd, _pi32]),
@@ -192,6 +194,9 @@ class DG:
         self._ck(_lib.dg_set_exterior(self._h, _ptr(ext, _pd)))
 
     # ---- RTM
+    def rtm_set_receiver_capacity(self, max_receivers):
+        self._ck(_lib.rtm_set_receiver_capacity(self._h, int(max_receivers)))
+
     def rtm_history_bytes(self, nsteps):
         n = _sz()
         self._ck(_lib.rtm_history_bytes(self._h, int(nsteps), C.byref(n)))
@@ -228,6 +233,21 @@ class DG:
 
     def rtm_image_zero(self):
         self._ck(_lib.rtm_image_zero(self._h))
+
+    def rtm_image_device(self):
+        """(device pointer, bytes) of the image in the blocked device layout."""
+        p, n = _vp(), _sz()
+        self._ck(_lib.rtm_image_device(self._h, C.byref(p), C.byref(n)))
+        return p.value, n.value
+
+    def image_torch(self):
+        """The device image as a 1-D torch view (float32 / float64) of the bound history tensor, for in-place
+        collectives across replicas (argument marshalling only: no arithmetic happens here)."""
+        import torch
+        p, n = self.rtm_image_device()
+        off = p - self._hist.data_ptr()
+        assert 0 <= off and off + n <= self._hist.numel()
+        return self._hist[off:off + n].view(torch.float64 if self.precision == 64 else torch.float32)
 
     # ---- getters
     def dg_get_nodes(self):

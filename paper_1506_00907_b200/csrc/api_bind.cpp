@@ -73,9 +73,6 @@ void upload_tables(dg_ctx* c) {
       if (off + m.ptab.size() * 4 > blob.size()) throw ApiError(DG_ERR_UNSUPPORTED, "too many distinct face permutations");
       std::memcpy(&blob[off], m.ptab.data(), m.ptab.size() * 4);
       upload_raw(c, c->d_D3Q, blob.data(), blob.size());
-      const int ce = c->kt->pipe_set_const(blob.data(), c->stream);
-      if (ce != 0) throw ApiError(DG_ERR_CUDA, std::string("constant tables: ") + cudaGetErrorString((cudaError_t)ce));
-      sync_stream(c);
     }
     if (c->kt->tc) {     // tensor-core kernel: B tables in the canonical K-major no-swizzle layout, split hi / lo (TF32)
       const int K1 = c->kt->tc_K1, K2 = c->kt->tc_K2, NN = c->kt->tc_NN;
@@ -159,7 +156,6 @@ void upload_tables(dg_ctx* c) {
   upload_raw(c, c->wperm, wperm.data(), wperm.size() * 4);
 
   for (int l = 0; l < md.nlevels; ++l) {
-    upload_raw(c, c->d_coarse[l], md.coarse_nb[l].data(), md.coarse_nb[l].size() * 4);
     std::vector<int32_t> sf(md.stored[l].size());
     for (size_t x = 0; x < sf.size(); ++x) {
       const int32_t bi = md.stored[l][x];

@@ -256,7 +256,7 @@ int dg_mesh_create(dg_ctx** out, int N, int precision, int64_t K, int64_t Nv, co
     for (size_t i = 0; i < c->mesh.bc.size(); ++i)
       if (c->mesh.bc[i] == DG_BC_PRESCRIBED) c->has_prescribed = true;
     c->kt = get_kernel_table(N, precision);
-    for (int l = 0; l < kMaxLevels; ++l) { c->d_coarse[l] = nullptr; c->d_stored[l] = nullptr; c->rec[l] = nullptr; }
+    for (int l = 0; l < kMaxLevels; ++l) { c->d_stored[l] = nullptr; c->rec[l] = nullptr; }
     c->F.reset_history(); c->R.reset_history();
     if (const char* k = std::getenv("DGRTM_KERNEL")) { c->use_pipe = std::string(k) != "step"; c->use_tc = std::string(k) == "tc"; }
   } catch (const std::exception& e) {
@@ -295,6 +295,7 @@ int dg_set_integrator(dg_ctx* ctx, int integrator) {
   if (integrator != DG_INTEGRATOR_AB3 && integrator != DG_INTEGRATOR_LSERK4) throw ApiError(DG_ERR_ARG, "unknown integrator");
   if (integrator == DG_INTEGRATOR_LSERK4 && ctx->has_model && ctx->model.nlevels != 1)
     throw ApiError(DG_ERR_UNSUPPORTED, "LSERK4 is single-rate only");
+  if (integrator != ctx->integrator && ctx->bound) restart_history(ctx);
   ctx->integrator = integrator;
   DG_CATCH(ctx)
 }
@@ -303,9 +304,23 @@ int dg_set_dt(dg_ctx* ctx, double dt_local) {
   DG_TRY(ctx)
   if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
   if (!(dt_local > 0)) throw ApiError(DG_ERR_ARG, "dt_local must be positive");
+  if (ctx->bound) restart_history(ctx);
   ctx->dt_local = dt_local;
   DG_CATCH(ctx)
 }
+
+} // extern C
+namespace dgrtm {
+// A change of integrator or step size invalidates the stored right-hand sides (LSERK4 uses hist[0] as stage scratch;
+// AB weights assume equal spacing): the time base moves to the current time and AB restarts with AB1, AB2 (reading Q7).
+void restart_history(dg_ctx* c) {
+  normalize_traces(c, c->F);
+  c->t0 = c->t0 + (double)c->fine * c->dt_local;
+  c->fine = 0;
+  c->F.reset_history();
+}
+}  // namespace dgrtm
+extern "C" {
 
 static void point_weights(dg_ctx* c, const double x[3], int64_t* k, double* row, double* w) {
   double rst[3];
@@ -347,7 +362,10 @@ int dg_set_receivers(dg_ctx* ctx, int64_t nr, const double* xr) {
     rk[r] = (int32_t)k;
   }
   ctx->nr = nr; ctx->rcv_k.swap(rk); ctx->rcv_row.swap(row); ctx->rcv_w.swap(w);
-  ctx->hist_bound = false;
+  // within the receiver capacity of the bound RTM region the region stays: image, q(t_f) and the trace history are
+  // untouched and only the receiver tables are replaced (gathers of a survey stack in place)
+  if (ctx->hist_bound && ctx->bound && nr <= ctx->nr_cap) upload_receiver_tables(ctx);
+  else ctx->hist_bound = false;
   DG_CATCH(ctx)
 }
 
@@ -385,8 +403,14 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
   c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);
   c->d_src_w = cv.take((size_t)Np * rs);
   for (int l = 0; l < md.nlevels; ++l) {
-    c->d_coarse[l] = (int*)cv.take(std::max<size_t>(1, md.coarse_nb[l].size()) * 4);
     c->d_stored[l] = (int*)cv.take(std::max<size_t>(1, md.stored[l].size()) * 4);
+  }
+}
+void check_launches(dg_ctx* c) {
+  cuda_check(cudaGetLastError(), "kernel launch");
+  if (c->kt && c->kt->take_error) {
+    const int e = c->kt->take_error();
+    if (e != 0) throw ApiError(DG_ERR_CUDA, std::string("cudaLaunchKernelEx: ") + cudaGetErrorString((cudaError_t)e));
   }
 }
 void require_bound(dg_ctx* c) {
@@ -405,13 +429,13 @@ int dg_workspace_bytes(dg_ctx* ctx, size_t* n) {
     OpsDev ops = ctx->ops; char* geo = ctx->geo; int* nbr = ctx->nbr; int* wperm = ctx->wperm; Field F = ctx->F;
     char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w;
     char* dp = ctx->d_D3P; char* lp = ctx->d_LTP; char* dq = ctx->d_D3Q; char* lq = ctx->d_LTQ; unsigned char* bf = ctx->d_blkflag; int* ps = ctx->d_pt_src;
-    int* dc[kMaxLevels]; int* ds[kMaxLevels];
-    for (int l = 0; l < kMaxLevels; ++l) { dc[l] = ctx->d_coarse[l]; ds[l] = ctx->d_stored[l]; }
+    int* ds[kMaxLevels];
+    for (int l = 0; l < kMaxLevels; ++l) ds[l] = ctx->d_stored[l];
     carve_workspace(ctx, count);
     ctx->ops = ops; ctx->geo = geo; ctx->nbr = nbr; ctx->wperm = wperm; ctx->F = F;
     ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw;
     ctx->d_D3P = dp; ctx->d_LTP = lp; ctx->d_D3Q = dq; ctx->d_LTQ = lq; ctx->d_blkflag = bf; ctx->d_pt_src = ps;
-    for (int l = 0; l < kMaxLevels; ++l) { ctx->d_coarse[l] = dc[l]; ctx->d_stored[l] = ds[l]; }
+    for (int l = 0; l < kMaxLevels; ++l) ctx->d_stored[l] = ds[l];
   }
   *n = count.used;
   DG_CATCH(ctx)

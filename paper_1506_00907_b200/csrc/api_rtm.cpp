@@ -39,7 +39,7 @@ void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
   const int Np = c->Np;
   for (int l = 0; l < md.nlevels; ++l)
     c->rec[l] = cv.take((size_t)records_of_level(c, l, nsteps) * md.stored[l].size() * c->REC * rs);
-  const size_t nr = (size_t)std::max<int64_t>(1, c->nr);
+  const size_t nr = (size_t)std::max<int64_t>(1, std::max(c->nr, c->nr_reserve));   // receiver capacity
   c->d_data = cv.take(nr * ((size_t)nsteps * c->nlocal + 1) * rs);
   c->d_rcv_slot = (int*)cv.take(nr * 4);
   c->d_rcv_level = (int*)cv.take(nr * 4);
@@ -107,7 +107,49 @@ void copy_data(dg_ctx* c, double* host, const double* host_in, int64_t ncol) {
 
 }  // namespace
 
+namespace dgrtm {
+void upload_receiver_tables(dg_ctx* ctx) {
+  group_receivers(ctx);
+  const int64_t nr = ctx->nr;
+  if (nr) {
+    std::vector<int32_t> slot(nr), lvl(nr);
+    for (int64_t r = 0; r < nr; ++r) {
+      slot[r] = (int32_t)ctx->model.slot_of[ctx->rcv_k[r]];
+      lvl[r] = ctx->model.level[ctx->rcv_k[r]];
+    }
+    upload_raw(ctx, ctx->d_rcv_slot, slot.data(), nr * 4);
+    upload_raw(ctx, ctx->d_rcv_level, lvl.data(), nr * 4);
+    upload_real(ctx, ctx->d_rcv_row, ctx->rcv_row.data(), ctx->rcv_row.size());
+    upload_real(ctx, ctx->d_rcv_w, ctx->rcv_w.data(), ctx->rcv_w.size());
+    upload_raw(ctx, ctx->d_grp_slot, ctx->grp_slot.data(), ctx->grp_slot.size() * 4);
+    upload_raw(ctx, ctx->d_grp_off, ctx->grp_off.data(), ctx->grp_off.size() * 4);
+    upload_raw(ctx, ctx->d_grp_rcv, ctx->grp_rcv.data(), ctx->grp_rcv.size() * 4);
+  }
+  std::vector<int32_t> idx((size_t)ctx->model.nslots, -1);
+  for (size_t g = 0; g < ctx->grp_slot.size(); ++g) idx[ctx->grp_slot[g]] = (int32_t)g;
+  upload_raw(ctx, ctx->d_pt_rcv, idx.data(), idx.size() * 4);
+  ctx->data_valid = false;
+}
+}  // namespace dgrtm
+
 extern "C" {
+
+int rtm_set_receiver_capacity(dg_ctx* ctx, int64_t max_receivers) {
+  DG_TRY(ctx)
+  if (max_receivers < 0) throw ApiError(DG_ERR_ARG, "max_receivers must be >= 0");
+  ctx->nr_reserve = max_receivers;
+  DG_CATCH(ctx)
+}
+
+int rtm_image_device(dg_ctx* ctx, void** dptr, size_t* nbytes) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (!dptr || !nbytes) throw ApiError(DG_ERR_ARG, "dptr / nbytes is NULL");
+  sync_stream(ctx);
+  *dptr = ctx->image;
+  *nbytes = (size_t)ctx->model.nblocks * ctx->Np * 32 * ctx->rs;
+  DG_CATCH(ctx)
+}
 
 int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n) {
   DG_TRY(ctx)
@@ -148,28 +190,8 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
   Carver cv;
   cv.base = ctx->hs;
   carve_history(ctx, cv, nsteps);
-  // receiver tables
-  group_receivers(ctx);
-  const int64_t nr = ctx->nr;
-  if (nr) {
-    std::vector<int32_t> slot(nr), lvl(nr);
-    for (int64_t r = 0; r < nr; ++r) {
-      slot[r] = (int32_t)ctx->model.slot_of[ctx->rcv_k[r]];
-      lvl[r] = ctx->model.level[ctx->rcv_k[r]];
-    }
-    upload_raw(ctx, ctx->d_rcv_slot, slot.data(), nr * 4);
-    upload_raw(ctx, ctx->d_rcv_level, lvl.data(), nr * 4);
-    upload_real(ctx, ctx->d_rcv_row, ctx->rcv_row.data(), ctx->rcv_row.size());
-    upload_real(ctx, ctx->d_rcv_w, ctx->rcv_w.data(), ctx->rcv_w.size());
-    upload_raw(ctx, ctx->d_grp_slot, ctx->grp_slot.data(), ctx->grp_slot.size() * 4);
-    upload_raw(ctx, ctx->d_grp_off, ctx->grp_off.data(), ctx->grp_off.size() * 4);
-    upload_raw(ctx, ctx->d_grp_rcv, ctx->grp_rcv.data(), ctx->grp_rcv.size() * 4);
-  }
-  {
-    std::vector<int32_t> idx((size_t)ctx->model.nslots, -1);
-    for (size_t g = 0; g < ctx->grp_slot.size(); ++g) idx[ctx->grp_slot[g]] = (int32_t)g;
-    upload_raw(ctx, ctx->d_pt_rcv, idx.data(), idx.size() * 4);
-  }
+  ctx->nr_cap = std::max(ctx->nr, ctx->nr_reserve);
+  upload_receiver_tables(ctx);
   ctx->hist_bound = true;
   clear_field(ctx, ctx->R);
   cuda_check(cudaMemsetAsync(ctx->image, 0, (size_t)ctx->model.nblocks * ctx->Np * 32 * ctx->rs, ctx->stream), "memset image");
@@ -191,8 +213,9 @@ int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out) {
   run_mrab(ctx, nsteps, o);
   ctx->fine = (int64_t)nsteps * ctx->nlocal;
   cuda_check(cudaMemcpyAsync(ctx->qfinal, ctx->F.q, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "save final state");
-  cuda_check(cudaGetLastError(), "kernel launch");
+  check_launches(ctx);
   ctx->have_final = true; ctx->final_nsteps = nsteps; ctx->have_backward = false;
+  ctx->data_valid = ctx->nr > 0;
   if (data_out) copy_data(ctx, data_out, nullptr, (int64_t)nsteps * ctx->nlocal + 1);
   sync_stream(ctx);
   DG_CATCH(ctx)
@@ -207,6 +230,9 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
   if (!updir) throw ApiError(DG_ERR_ARG, "updir is NULL");
   if (imaging < 0 || imaging > 3) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
   const int64_t ntot = ctx->final_nsteps;
+  if (!data && ctx->nr > 0 && !ctx->data_valid)
+    throw ApiError(DG_ERR_STATE, "the signals on the device belong to another receiver set: pass data");
+  if (data) ctx->data_valid = true;
   if (data) copy_data(ctx, nullptr, data, ntot * ctx->nlocal + 1);   // NULL: the signals recorded on the device
   // source field: restart from q(t_f) (history restarts, reading Q7); receiver field: from rest
   cuda_check(cudaMemcpyAsync(ctx->F.q, ctx->qfinal, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "restore final state");
@@ -225,7 +251,7 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
   o.t0 = (double)ntot * ((double)ctx->nlocal * ctx->dt_local);
   run_mrab(ctx, nsteps, o);
   ctx->fine = (ntot - nsteps) * ctx->nlocal;
-  cuda_check(cudaGetLastError(), "kernel launch");
+  check_launches(ctx);
   ctx->have_backward = true;
   sync_stream(ctx);
   DG_CATCH(ctx)

@@ -11,48 +11,6 @@ namespace {
 
 inline int lvl_blk_end(const Model& md, int l) { return md.lvl_blk0[l] + md.lvl_nblk[l]; }
 
-void launch_update(dg_ctx* c, Field& F, int l, double dts) {
-  const AbCoef& co = ab_coef(F.nhist[l]);
-  UpdateArgs u;
-  std::memset(&u, 0, sizeof(u));
-  u.q = F.q; u.qf = F.qf; u.h0 = F.h(l, 0); u.h1 = F.h(l, 1); u.h2 = F.h(l, 2);
-  u.geo = c->geo; u.wperm = c->wperm;
-  u.blk0 = c->model.lvl_blk0[l]; u.nblk = c->model.lvl_nblk[l];
-  u.c0 = dts * co.a[0]; u.c1 = dts * co.a[1]; u.c2 = dts * co.a[2];      // eq (18)
-  u.ops = c->ops;
-  if (u.nblk > 0) DG_LAUNCH(c, KC_UPDATE, c->kt->update(u, c->stream));
-}
-
-void launch_half(dg_ctx* c, Field& F, int l, double dts) {
-  const int n = (int)c->model.coarse_nb[l].size();
-  if (!n) return;
-  const AbCoef& co = ab_coef(F.nhist[l]);
-  HalfArgs h;
-  std::memset(&h, 0, sizeof(h));
-  h.q = F.q; h.qf = F.qf; h.h0 = F.h(l, 0); h.h1 = F.h(l, 1); h.h2 = F.h(l, 2);
-  h.geo = c->geo; h.wperm = c->wperm; h.list = c->d_coarse[l]; h.nlist = n;
-  h.c0 = dts * co.b[0]; h.c1 = dts * co.b[1]; h.c2 = dts * co.b[2];      // eq (19)
-  h.ops = c->ops;
-  DG_LAUNCH(c, KC_HALF, c->kt->half(h, c->stream));
-}
-
-void launch_image_update(dg_ctx* c, Field& S, Field& R, int l, double dts, const RunOpts& o) {
-  const AbCoef& co = ab_coef(S.nhist[l]);
-  ImageArgs a;
-  std::memset(&a, 0, sizeof(a));
-  a.qS = S.q; a.qfS = S.qf; a.hS0 = S.h(l, 0); a.hS1 = S.h(l, 1); a.hS2 = S.h(l, 2);
-  a.qR = R.q; a.qfR = R.qf; a.hR0 = R.h(l, 0); a.hR1 = R.h(l, 1); a.hR2 = R.h(l, 2);
-  a.image = c->image; a.geo = c->geo; a.wperm = c->wperm;
-  a.blk0 = c->model.lvl_blk0[l]; a.nblk = c->model.lvl_nblk[l];
-  a.dts = dts;
-  for (int s = 0; s < 3; ++s) { a.a[s] = co.a[s]; a.abar[s] = co.abar[s]; }
-  for (int s = 0; s < 9; ++s) a.C[s] = co.C[s];
-  for (int d = 0; d < 3; ++d) a.e[d] = o.updir[d];
-  a.characteristic = o.imaging == DG_IMAGING_CHARACTERISTIC;
-  a.ops = c->ops;
-  if (a.nblk > 0) DG_LAUNCH(c, KC_IMAGE, c->kt->image_update(a, c->stream));
-}
-
 PointArgs point_args(dg_ctx* c, const Field& F) {
   PointArgs p;
   std::memset(&p, 0, sizeof(p));
@@ -257,7 +215,7 @@ int dg_step(dg_ctx* ctx, int nsteps) {
     run_mrab(ctx, nsteps, o);
     ctx->fine += (int64_t)nsteps * ctx->nlocal;
   }
-  cuda_check(cudaGetLastError(), "kernel launch");
+  check_launches(ctx);
   DG_CATCH(ctx)
 }
 
@@ -278,7 +236,7 @@ int dg_get_rhs(dg_ctx* ctx, int which, int direction, double* r) {
   cuda_check(cudaMemsetAsync(ctx->scratch, 0, field_bytes(ctx), ctx->stream), "memset scratch");
   normalize_traces(ctx, ctx->F);
   launch_rhs(ctx, ctx->F, ctx->scratch, 0, ctx->model.nlevels, mode, (double)direction, nullptr, nullptr);
-  cuda_check(cudaGetLastError(), "kernel launch");
+  check_launches(ctx);
   fields_from_device(ctx, r, ctx->scratch);
   DG_CATCH(ctx)
 }
@@ -350,7 +308,7 @@ int dg_bench_kernel(dg_ctx* ctx, int which, int reps) {
       default: throw ApiError(DG_ERR_ARG, "which must be 0..4");
     }
   }
-  cuda_check(cudaGetLastError(), "kernel launch");
+  check_launches(ctx);
   DG_CATCH(ctx)
 }
 

@@ -101,6 +101,9 @@ struct dg_ctx {
   double f0 = 0, tp = 0, amp = 0;
   // receivers
   int64_t nr = 0;
+  int64_t nr_reserve = 0;                   // rtm_set_receiver_capacity
+  int64_t nr_cap = 0;                       // receiver capacity of the bound RTM region
+  bool data_valid = false;                  // d_data holds signals of the current receiver set
   std::vector<int32_t> rcv_k;
   std::vector<double> rcv_row, rcv_w;
   std::vector<int32_t> grp_slot, grp_off, grp_rcv;   // receivers grouped by element, groups by level
@@ -128,7 +131,6 @@ struct dg_ctx {
   bool use_tc = false;                      // DGRTM_KERNEL=tc selects the tensor-core kernel (fp32, one wavefield)
   unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
-  int* d_coarse[dgrtm::kMaxLevels];         // per level: slots with a finer face neighbour
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
   int64_t fine = 0;                         // time = t0 + fine * dt_local
@@ -178,6 +180,8 @@ void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
 void normalize_traces(dg_ctx* c, Field& F);
 void upload_point_source(dg_ctx* c);        // per-slot point-term index of the forward field // current traces of every level -> qfb[0] (= qf)
 void clear_field(dg_ctx* c, Field& F);
+void upload_receiver_tables(dg_ctx* c);     // receiver rows / weights / groups -> the bound RTM region
+void restart_history(dg_ctx* c);            // after dg_set_integrator / dg_set_dt
 
 struct RunOpts {
   int direction = 1;
@@ -199,6 +203,7 @@ void launch_rhs(dg_ctx* c, Field& F, char* out, int l0, int l1, int mode, double
                 const char* replay);
 void carve_workspace(dg_ctx* c, Carver& cv);
 void require_bound(dg_ctx* c);
+void check_launches(dg_ctx* c);             // cudaGetLastError + the first failed dependent launch, as DG_ERR_CUDA
 
 // counts a launch and, in profiling mode, brackets it with an event pair on the bound stream
 struct LaunchScope {

@@ -8,7 +8,6 @@
 //                  incl. boundary-trace capture / replay
 //   k_update       AB update (18) + exposed traces (Alg. 4)
 //   k_rk           LSERK4 stage (reading Q8)
-//   k_half         half-step traces (19) of coarse neighbours (Alg. 1)
 //   k_image_update backward update of source + receiver fields fused with the image contribution
 //                  (eqs (7)-(8) PAPER.md:61-65, (20)-(24) PAPER.md:174-204, readings Q1, Q1b)
 //   k_source / k_record / k_inject   point terms (eq (15))
@@ -402,38 +401,6 @@ __global__ void __launch_bounds__(32 * Tiling<N>::T) k_image_update(ImageArgs a)
     write_traces<real, N>(static_cast<real*>(a.qfR), stR, b, 32 * T);
     __syncthreads();
   }
-}
-
-// -------------------------------------------------------------------------------------------------
-// half-step traces (19): thread = (face node j, list entry e), e fastest
-template <typename real, int N>
-__global__ void k_half(HalfArgs a) {
-  using O = Order<N>;
-  constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, REC = O::REC;
-  const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (tid >= (long)a.nlist * NF) return;
-  const int j = (int)(tid / a.nlist), e = (int)(tid - (long)j * a.nlist);
-  const int slot = a.list[e], b = slot >> 5, lane = slot & 31;
-  const int f = j / Nfp, i = j - f * Nfp, n = a.ops.Fmask[j];
-  const real* q = static_cast<const real*>(a.q);
-  const real* h0 = static_cast<const real*>(a.h0);
-  const real* h1 = static_cast<const real*>(a.h1);
-  const real* h2 = static_cast<const real*>(a.h2);
-  const real* geo = static_cast<const real*>(a.geo);
-  const real c0 = (real)a.c0, c1 = (real)a.c1, c2 = (real)a.c2;
-  real v[4];
-#pragma unroll
-  for (int fld = 0; fld < 4; ++fld) {
-    const size_t o = (size_t)b * (4 * Np * 32) + (size_t)(fld * Np + n) * 32 + lane;
-    v[fld] = q[o] + (c0 * h0[o] + c1 * h1[o] + c2 * h2[o]);
-  }
-  const real* gf = geo + ((size_t)b * DG_NGEO + GEO_FACE + 5 * f) * 32 + lane;
-  const real nv = gf[0] * v[1] + gf[32] * v[2] + gf[64] * v[3];
-  const int wp = a.wperm[slot];
-  const int pos = a.ops.ptab[((wp >> (8 * f)) & 255) * Nfp + i];
-  real* rec = static_cast<real*>(a.qf) + ((size_t)slot * 4 + f) * REC;
-  rec[pos] = v[0];
-  rec[Nfp + pos] = nv;
 }
 
 // own traces of listed boundary faces -> history record (final time, reading Q12)

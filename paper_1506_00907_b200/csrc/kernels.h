@@ -61,13 +61,6 @@ struct RkArgs {            // res = A res + dt r; q += B res (LSERK4, reading Q8
   OpsDev ops;
 };
 
-struct HalfArgs {          // traces of q + c0 h0 + c1 h1 + c2 h2 (eq (19)) for a list of slots
-  const void* q; void* qf; const void* h0; const void* h1; const void* h2;
-  const void* geo; const int* wperm; const int* list; int nlist;
-  double c0, c1, c2;
-  OpsDev ops;
-};
-
 struct ImageArgs {         // backward update of two wavefields with the imaging contribution (24)
   void* qS; void* qfS; const void* hS0; const void* hS1; const void* hS2;
   void* qR; void* qfR; const void* hR0; const void* hR1; const void* hR2;
@@ -146,7 +139,6 @@ struct KernelTable {
   void (*rhs)(const RhsArgs&, cudaStream_t);
   void (*update)(const UpdateArgs&, cudaStream_t);
   void (*rk)(const RkArgs&, cudaStream_t);
-  void (*half)(const HalfArgs&, cudaStream_t);
   void (*image_update)(const ImageArgs&, cudaStream_t);
   void (*source)(const PointArgs&, cudaStream_t);
   void (*record)(const PointArgs&, cudaStream_t);
@@ -159,13 +151,13 @@ struct KernelTable {
   void (*pipe)(const StepArgs&, cudaStream_t);
   void (*pipe2)(const StepArgs&, cudaStream_t);
   int pipe_TO, pipe_NT, pipe_RL, pipe_LL;
-  size_t pipe_blob_bytes;
-  int (*pipe_set_const)(const void* blob_host, cudaStream_t);
+  size_t pipe_blob_bytes;                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
   // tensor-core variant (tc_kernel.cuh; fp32, one wavefield); tc == nullptr if not instantiated
   void (*tc)(const StepArgs&, cudaStream_t);
   int tc_K1, tc_K2, tc_NN;
-  size_t tc_blob_bytes;                                // [B1 hi | B1 lo | B2 hi | B2 lo | Fmask | perm table]   // operator part of the blob -> constant memory                              // [D3Q | LTQ | Fmask | perm table], the kernel's table image
-  int (*init)();           // sets shared-memory attributes; returns cudaError
+  size_t tc_blob_bytes;                                // [B1 hi | B1 lo | B2 hi | B2 lo | Fmask | perm table]
+  int (*init)();           // sets shared-memory attributes, reads the device's SM count; returns cudaError
+  int (*take_error)();     // first error of a programmatic-dependent launch since the last call (cudaError), then cleared
 };
 
 const KernelTable* get_kernel_table(int N, int precision);

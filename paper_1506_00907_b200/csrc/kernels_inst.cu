@@ -9,7 +9,8 @@ namespace dgrtm {
 namespace {
 
 constexpr int N = DG_ORDER;
-constexpr int kSMs = 148;   // B200
+int g_sms = 148;            // B200; replaced by the current device's SM count in Launch::init()
+cudaError_t g_launch_error = cudaSuccess;   // first failed cudaLaunchKernelEx (reported by Launch::take_error)
 
 template <typename F> int blocks_per_sm(F kernel, int threads, size_t smem) {
   int n = 0;
@@ -18,7 +19,7 @@ template <typename F> int blocks_per_sm(F kernel, int threads, size_t smem) {
 }
 
 inline int persistent_grid(int nblk, int per_sm) {
-  const int cap = kSMs * per_sm;
+  const int cap = g_sms * per_sm;
   return nblk < cap ? nblk : cap;
 }
 
@@ -33,14 +34,22 @@ void launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_t s, co
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, kernel, a);
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, a);
+  if (e != cudaSuccess && g_launch_error == cudaSuccess) g_launch_error = e;
 }
 
 template <typename real> struct Launch {
   static int occ_rhs, occ_upd, occ_rk, occ_img;
 
+  static int take_error() { const int e = (int)g_launch_error; g_launch_error = cudaSuccess; return e; }
   static int init() {
     cudaError_t e;
+    int dev = 0, sms = 0;
+    e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return (int)e;
+    if (sms > 0) g_sms = sms;
     e = cudaFuncSetAttribute(k_rhs<real, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RhsSmem<real, N>::bytes);
     if (e != cudaSuccess) return (int)e;
     e = cudaFuncSetAttribute(k_update<real, N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -87,11 +96,6 @@ template <typename real> struct Launch {
     if (a.nblk <= 0) return;
     k_update<real, N, 1><<<persistent_grid(a.nblk, occ_rk), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(1), s>>>(UpdateArgs(), a);
   }
-  static void half(const HalfArgs& a, cudaStream_t s) {
-    if (a.nlist <= 0) return;
-    const long n = (long)a.nlist * Order<N>::NF;
-    k_half<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
-  }
   static void image_update(const ImageArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     k_image_update<real, N><<<persistent_grid(a.nblk, occ_img), 32 * Tiling<N>::T, UpdSmem<N>::template bytes<real>(2), s>>>(a);
@@ -99,36 +103,28 @@ template <typename real> struct Launch {
   static void step(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using SM = StepSmem<real, N, false>;
-    k_step<real, N, false><<<a.nblk < kSMs ? a.nblk : kSMs, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
+    k_step<real, N, false><<<a.nblk < g_sms ? a.nblk : g_sms, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
   }
   static void step2(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using SM = StepSmem<real, N, true>;
-    k_step<real, N, true><<<a.nblk < kSMs ? a.nblk : kSMs, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
+    k_step<real, N, true><<<a.nblk < g_sms ? a.nblk : g_sms, SM::G * StepCfg<real, N>::NT * 32, SM::bytes, s>>>(a);
   }
   static void pipe(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    launch_pdl(k_pipe<real, N, false>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    launch_pdl(k_pipe<real, N, false>, a.nblk < g_sms ? a.nblk : g_sms, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void pipe2(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    launch_pdl(k_pipe<real, N, true>, a.nblk < kSMs ? a.nblk : kSMs, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    launch_pdl(k_pipe<real, N, true>, a.nblk < g_sms ? a.nblk : g_sms, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void tc(const StepArgs& a, cudaStream_t s) {
     if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled) {
       if (a.nblk <= 0) return;
-      launch_pdl(k_tc<N>, a.nblk < kSMs ? a.nblk : kSMs, TcCfg<N>::G * 128, TcSmem<N>::bytes, s, a);
+      launch_pdl(k_tc<N>, a.nblk < g_sms ? a.nblk : g_sms, TcCfg<N>::G * 128, TcSmem<N>::bytes, s, a);
     }
-  }
-  static int pipe_set_const(const void* blob_host, cudaStream_t s) {
-    if constexpr (PipeCfg<real, N>::enabled) {
-      const size_t n = PipeSmem<real, N>::ops_reals * sizeof(real);
-      if constexpr (sizeof(real) == 4) return (int)cudaMemcpyToSymbolAsync(c_pipe_ops_f, blob_host, n, 0, cudaMemcpyHostToDevice, s);
-      else return (int)cudaMemcpyToSymbolAsync(c_pipe_ops_d, blob_host, n, 0, cudaMemcpyHostToDevice, s);
-    }
-    return 0;
   }
   static void source(const PointArgs& a, cudaStream_t s) { k_source<real, N><<<1, 96, 0, s>>>(a); }
   static void record(const PointArgs& a, cudaStream_t s) {
@@ -155,10 +151,10 @@ template <typename real> KernelTable make_table(int precision) {
   KernelTable t;
   t.N = N; t.precision = precision; t.Np = Order<N>::Np; t.Nfp = Order<N>::Nfp;
   t.rhs = Launch<real>::rhs; t.update = Launch<real>::update; t.rk = Launch<real>::rk;
-  t.half = Launch<real>::half; t.image_update = Launch<real>::image_update;
+  t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
-  t.capture = Launch<real>::capture; t.init = Launch<real>::init;
-  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0; t.pipe_set_const = nullptr;
+  t.capture = Launch<real>::capture; t.init = Launch<real>::init; t.take_error = Launch<real>::take_error;
+  t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0;
   t.tc = nullptr; t.tc_K1 = t.tc_K2 = t.tc_NN = 0; t.tc_blob_bytes = 0;
   if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled && TcSmem<N>::fits) {
     t.tc = Launch<real>::tc; t.tc_K1 = TcSmem<N>::K1; t.tc_K2 = TcSmem<N>::K2; t.tc_NN = TcSmem<N>::NN;
@@ -168,7 +164,7 @@ template <typename real> KernelTable make_table(int precision) {
     t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
     t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;
     t.pipe_RL = PipeSmem<real, N>::RL; t.pipe_LL = PipeSmem<real, N>::LL;
-    t.pipe_blob_bytes = PipeSmem<real, N>::ops_bytes; t.pipe_set_const = Launch<real>::pipe_set_const;
+    t.pipe_blob_bytes = PipeSmem<real, N>::ops_bytes;
   }
   t.step = Launch<real>::step; t.step2 = Launch<real>::step2; t.step_npad = StepSmem<real, N, false>::NPAD;
   return t;

@@ -60,7 +60,10 @@ template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; sta
 #ifndef DG_P4_UG
 #define DG_P4_UG 1
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = 1, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0; };
+#ifndef DG_P4_QS
+#define DG_P4_QS 1
+#endif
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
@@ -112,104 +115,6 @@ __device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&o
     for (int e = 0; e < VW; ++e) out[v * VW + e] = xs[e];
   }
 }
-
-// ---- operator tables in constant memory: with the tile index and all loop indices known at compile time
-// every operator entry becomes a c[bank][offset] operand of its FFMA / DFMA: no shared-memory traffic and
-// no load instruction for the operators (one table per translation unit = per order).
-// MEASURED (B200, N = 3 fp32, cfg2): ptxas turns the entries into LDCU.128 -> uniform registers -> FFMA R,R,UR,R;
-// the 10 KB table streams through the small constant cache and the step slows from 66 to 112 us (N = 4: 3.1x
-// slower).  Kept as a compile-time option (-DDG_PIPE_COPS=1), off by default; see DESIGN.md.
-#ifndef DG_PIPE_COPS
-#define DG_PIPE_COPS 0
-#endif
-#ifdef DG_ORDER
-__constant__ float c_pipe_ops_f[PipeCfg<float, DG_ORDER>::enabled ? PipeSmem<float, DG_ORDER>::ops_reals : 1];
-__constant__ double c_pipe_ops_d[PipeCfg<double, DG_ORDER>::enabled ? PipeSmem<double, DG_ORDER>::ops_reals : 1];
-template <typename real> struct PipeConst;
-template <> struct PipeConst<float> { static __device__ __forceinline__ const float* ops() { return c_pipe_ops_f; } };
-template <> struct PipeConst<double> { static __device__ __forceinline__ const double* ops() { return c_pipe_ops_d; } };
-
-// volume + surface of output tile TILE (= warp w of the group) with constant-bank operators
-template <typename real, int N, int TILE>
-__device__ __forceinline__ void pipe_tile_const(const real* __restrict__ Q, const real* __restrict__ pen, const real* __restrict__ geo,
-                                                int lane, int g, real rc2, real irho, const real (&gm)[9],
-                                                real (&rp)[PipeCfg<real, N>::TO], real (&rx)[PipeCfg<real, N>::TO],
-                                                real (&ry)[PipeCfg<real, N>::TO], real (&rz)[PipeCfg<real, N>::TO]) {
-  using O = Order<N>;
-  using Cfg = PipeCfg<real, N>;
-  using SM = PipeSmem<real, N>;
-  constexpr int Np = O::Np, Nfp = O::Nfp, NF = O::NF, TO = Cfg::TO, NT = Cfg::NT, RL = SM::RL, LL = SM::LL, VW = SM::VW, PV = SM::PV;
-  constexpr bool INPLACE = NT > 1 && Cfg::UG;
-  const real* cD = PipeConst<real>::ops() + (size_t)TILE * Np * RL;
-  const real* cL = PipeConst<real>::ops() + (size_t)NT * Np * RL + (size_t)TILE * NF * LL;
-  real aD[TO], aR[TO], aS[TO], aT[TO];
-#pragma unroll
-  for (int nn = 0; nn < TO; ++nn) { aD[nn] = 0; aR[nn] = 0; aS[nn] = 0; aT[nn] = 0; }
-#pragma unroll
-  for (int m = 0; m < Np; ++m) {
-    const real p = Q[m * 32 + lane];
-    real ur, us, ut;
-    if (INPLACE) {
-      ur = Q[(Np + m) * 32 + lane]; us = Q[(2 * Np + m) * 32 + lane]; ut = Q[(3 * Np + m) * 32 + lane];
-    } else {
-      const real vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
-      ur = gm[0] * vx + gm[3] * vy + gm[6] * vz; us = gm[1] * vx + gm[4] * vy + gm[7] * vz; ut = gm[2] * vx + gm[5] * vy + gm[8] * vz;
-    }
-#pragma unroll
-    for (int nn = 0; nn < TO; ++nn) {
-      const real dr = cD[m * RL + nn], ds = cD[m * RL + TO + nn], dt = cD[m * RL + 2 * TO + nn];
-      aD[nn] = fma(dr, ur, aD[nn]); aD[nn] = fma(ds, us, aD[nn]); aD[nn] = fma(dt, ut, aD[nn]);
-      aR[nn] = fma(dr, p, aR[nn]); aS[nn] = fma(ds, p, aS[nn]); aT[nn] = fma(dt, p, aT[nn]);
-    }
-  }
-#pragma unroll
-  for (int nn = 0; nn < TO; ++nn) {
-    rp[nn] = -rc2 * aD[nn];
-    rx[nn] = -irho * (gm[0] * aR[nn] + gm[1] * aS[nn] + gm[2] * aT[nn]);
-    ry[nn] = -irho * (gm[3] * aR[nn] + gm[4] * aS[nn] + gm[5] * aT[nn]);
-    rz[nn] = -irho * (gm[6] * aR[nn] + gm[7] * aS[nn] + gm[8] * aT[nn]);
-  }
-  group_sync<NT>(g);                          // every warp has read Q: the update may overwrite its tile's nodes
-#pragma unroll
-  for (int f = 0; f < 4; ++f) {
-    real av[TO];
-#pragma unroll
-    for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
-    real Ppv[PV * VW], Pvv[PV * VW];
-    {
-      using V = typename VecT<real, VW>::T;
-      const V* srcp = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 0) * PV) * 32 + lane;
-      const V* srcv = reinterpret_cast<const V*>(pen) + ((size_t)(f * 2 + 1) * PV) * 32 + lane;
-#pragma unroll
-      for (int v = 0; v < PV; ++v) {
-        *reinterpret_cast<V*>(&Ppv[v * VW]) = srcp[v * 32];
-        *reinterpret_cast<V*>(&Pvv[v * VW]) = srcv[v * 32];
-      }
-    }
-#pragma unroll
-    for (int i2 = 0; i2 < Nfp; ++i2) {
-      const int j = f * Nfp + i2;
-#pragma unroll
-      for (int nn = 0; nn < TO; ++nn) {
-        const real lv = cL[j * LL + nn];
-        rp[nn] = fma(-lv, Ppv[i2], rp[nn]); av[nn] = fma(lv, Pvv[i2], av[nn]);
-      }
-    }
-    const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
-#pragma unroll
-    for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
-  }
-}
-template <typename real, int N, int TILE>
-__device__ __forceinline__ void pipe_tile_dispatch(int w, const real* Q, const real* pen, const real* geo, int lane, int g, real rc2,
-                                                   real irho, const real (&gm)[9], real (&rp)[PipeCfg<real, N>::TO],
-                                                   real (&rx)[PipeCfg<real, N>::TO], real (&ry)[PipeCfg<real, N>::TO],
-                                                   real (&rz)[PipeCfg<real, N>::TO]) {
-  if (w == TILE) pipe_tile_const<real, N, TILE>(Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
-  else if constexpr (TILE + 1 < PipeCfg<real, N>::NT)
-    pipe_tile_dispatch<real, N, TILE + 1>(w, Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
-}
-#endif  // DG_ORDER
 
 template <typename real, int N, bool DUAL>
 __global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
@@ -500,12 +405,6 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- volume (eqs (13)-(14), Alg. 2)
     real rp[TO], rx[TO], ry[TO], rz[TO];
-#if DG_PIPE_COPS
-    {
-      const real gm[9] = {g00, g01, g02, g10, g11, g12, g20, g21, g22};
-      pipe_tile_dispatch<real, N, 0>(w, Q, pen, geo, lane, g, rc2, irho, gm, rp, rx, ry, rz);
-    }
-#else
     if constexpr (sizeof(real) == 4 && !DUAL && Cfg::F2) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
                                                  // (the two-field kernel is register-bound and keeps scalar FMAs)
       float2 aG2[RL / 2], aD2[RL / 2];
@@ -608,7 +507,6 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
     }
-#endif
 
     // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
     const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);

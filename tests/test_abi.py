@@ -47,6 +47,11 @@ def test_host_only_calls(lib_path):
     g.dg_set_model(np.ones(48), np.ones(48), 2, 0.15)
     assert g.dg_workspace_bytes() > 48 * 4 * 20 * 4 * 4
     assert g.rtm_history_bytes(10) > 0
+    n0 = g.rtm_history_bytes(10)
+    g.rtm_set_receiver_capacity(1000)                       # sizes the receiver-dependent part of the RTM region
+    assert g.rtm_history_bytes(10) > n0 + 1000 * 11 * 4
+    g.rtm_set_receiver_capacity(0)
+    assert g.rtm_history_bytes(10) == n0
     dt, nloc = g.dg_get_dt()
     assert dt > 0 and nloc == 2
     lv = g.dg_get_levels()

@@ -298,38 +298,49 @@ def test_rtm_trapezoid_imaging(precision, N, imaging, mode):
     g.close()
 
 
-def test_two_shot_survey_stacks_images():
+def test_survey_stacks_images_in_the_library():
     """several gathers over one mesh: the set-up (operators, geometry,
-    connectivity, levels) is reused, source and receivers change between shots, the images add up."""
+    connectivity, levels, device tables) is made once ("preparatory phase ... once for the complete survey",
+    PAPER.md:478), source and receiver set change between shots, and the images add up IN the library:
+    with a receiver capacity reserved, dg_set_receivers keeps the bound RTM region and its image."""
     nsteps = 24
     cfg = make_config("cfg4_rtm", hexes=(5, 4, 3), N=3, nsteps=nsteps, n_receivers_side=3)
     shots = [dict(x0=cfg["source"]["x0"], rcv=cfg["receivers"]),
-             dict(x0=cfg["source"]["x0"] + np.array([0.41, -0.33, 0.05]), rcv=cfg["receivers"][::2] + np.array([0.07, 0.03, 0.0]))]
-    g = make_gpu(cfg, 64)
-    I_sum = 0.0
-    for sh in shots:
-        c2 = dict(cfg, source=dict(cfg["source"], x0=sh["x0"], f0=60.0, tp=0.01), receivers=sh["rcv"])
-        o = make_oracle(c2)
-        data_o, hist, qT = o.rtm_forward(nsteps)
-        I_o, _, _ = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], nglobal_total=nsteps)
-        I_sum = I_sum + I_o
-        # the RTM region is sized by the receiver count: a new receiver set needs a new region, so the image so far is
-        # read out first and the stack continues on the host (same receiver set: no re-bind, the image stacks in place)
-        img = g.rtm_image_read() if g._hist is not None else None
-        g.dg_set_source(sh["x0"], 60.0, 0.01, 1.0)
-        g.dg_set_receivers(sh["rcv"])
+             dict(x0=cfg["source"]["x0"] + np.array([0.41, -0.33, 0.05]), rcv=cfg["receivers"][::2] + np.array([0.07, 0.03, 0.0])),
+             dict(x0=cfg["source"]["x0"] + np.array([-0.52, 0.27, 0.02]), rcv=cfg["receivers"][1::3] + np.array([-0.05, 0.04, 0.0]))]
+    for precision in (64, 32):
+        g = make_gpu(cfg, precision)
+        g.rtm_set_receiver_capacity(max(len(sh["rcv"]) for sh in shots))
         g.bind_history_torch(nsteps)
-        if img is not None:
-            assert np.abs(g.rtm_image_read()).max() == 0                  # a fresh history region starts from zero
-        data_g = g.rtm_forward_shot(nsteps)
-        assert rel_l2(data_g, data_o) < 1e-10
-        g.rtm_backward_shot(nsteps, data_o, updir=cfg["updir"])
-        if img is not None:
-            I_g = img + g.rtm_image_read()
-        else:
-            I_g = g.rtm_image_read()
-    assert rel_l2(I_g, I_sum) < 1e-10
-    g.close()
+        launches0 = g.dg_get_launch_count()
+        I_sum = 0.0
+        for n, sh in enumerate(shots):
+            c2 = dict(cfg, source=dict(cfg["source"], x0=sh["x0"], f0=60.0, tp=0.01), receivers=sh["rcv"])
+            o = make_oracle(c2)
+            data_o, hist, qT = o.rtm_forward(nsteps)
+            I_o, _, _ = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], nglobal_total=nsteps)
+            I_sum = I_sum + I_o
+            before = g.rtm_image_read()
+            g.dg_set_source(sh["x0"], 60.0, 0.01, 1.0)
+            g.dg_set_receivers(sh["rcv"])                                  # within the capacity: region and image stay
+            assert np.array_equal(g.rtm_image_read(), before)
+            if n == 1:                                                     # device signals now belong to another set
+                import paper_1506_00907_b200 as pk
+                with pytest.raises(pk.DGError) as e:
+                    g.rtm_backward_shot(nsteps, None, updir=cfg["updir"])
+                assert e.value.code == pk.DG_ERR_STATE
+            data_g = g.rtm_forward_shot(nsteps)
+            assert rel_l2(data_g, data_o) < TOL[precision]
+            g.rtm_backward_shot(nsteps, None if n == 2 else data_o, updir=cfg["updir"])   # NULL: the recorded signals
+            assert rel_l2(g.rtm_image_read(), I_sum) < (1e-10 if precision == 64 else 1e-4)
+        assert g.dg_get_launch_count() > launches0
+        # a receiver set beyond the capacity unbinds the region (the documented behaviour)
+        import paper_1506_00907_b200 as pk
+        g.dg_set_receivers(np.concatenate([cfg["receivers"], cfg["receivers"] + 0.01]))
+        with pytest.raises(pk.DGError) as e:
+            g.rtm_image_read()
+        assert e.value.code == pk.DG_ERR_STATE
+        g.close()
 
 
 def test_rtm_first_image_step():

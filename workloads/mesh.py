@@ -110,3 +110,17 @@ def permute_elements(etov, seed):
     rng = np.random.default_rng(seed)
     perm = rng.permutation(etov.shape[0])
     return np.ascontiguousarray(etov[perm]), perm
+
+
+def box_side_bc(etov, vx, lengths, top=1, bottom=3, sides=2):
+    """face_bc[K][4] (int8) of a box mesh by box side: faces on z = 0 get `top`, on z = Lz `bottom`, all others `sides`
+    (1 free surface, 2 absorbing, 3 rigid, 4 prescribed; only the entries of boundary faces are read by the solvers).
+    A face is assigned by the position of its centroid; local face f holds the vertices below (reference-element
+    convention shared by all users: F0 = {0,1,2}, F1 = {0,1,3}, F2 = {1,2,3}, F3 = {0,2,3})."""
+    faces = ((0, 1, 2), (0, 1, 3), (1, 2, 3), (0, 2, 3))
+    bc = np.full((etov.shape[0], 4), sides, dtype=np.int8)
+    for f, fv in enumerate(faces):
+        zc = vx[etov[:, fv]].mean(axis=1)[:, 2]
+        bc[zc < 1e-9 * lengths[2], f] = top
+        bc[zc > lengths[2] * (1 - 1e-9), f] = bottom
+    return bc
