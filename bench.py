@@ -1,6 +1,6 @@
 """bench.py - the headline measurement of the DGTD hot path (contract: DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2_two_layer]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2_two_layer|survey]
                     [--timesteps T] [--no-extras]
 
 One bench "step" = one whole pass of the hot path over one batch of synthetic input = T global time
@@ -15,6 +15,8 @@ cpu_baseline = the fp64 numpy oracle on the box's host cores on a bounded sample
 --impl reference times that oracle (there is no reference implementation: the reference is a paper).
 Multi-GPU (torchrun): the path has no inter-GPU step here ("replicas only"): every rank runs
 the same workload on its own GPU, value = total DOF-updates / max-over-ranks time, scaling = weak.
+--workload survey: a multi-shot survey over one mesh: the set-up is made once, the shots
+are split over the ranks, the images stack in the library, and ONE all-reduce of the image (outside the step) ends it.
 """
 import argparse
 import json
@@ -47,6 +49,21 @@ def parse_args():
     ap.add_argument("--hexes", default="", help="nx,ny,nz override (development)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline and the per-config extras")
     return ap.parse_args()
+
+
+def load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+    (profiles/ncu_traffic.json, written from the captures; key "workload|N|precision|kernel")."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(p):
+        return {}
+    with open(p) as fh:
+        return {k: v for k, v in json.load(fh).items() if not k.startswith("_")}
+
+
+def traffic_of(table, workload, N, precision, kernel):
+    e = table.get("%s|%d|%d|%s" % (workload, N, precision, kernel))
+    return None if e is None else int(e["dram_bytes_per_launch"])
 
 
 def load_peaks():
@@ -194,7 +211,7 @@ def timed_steps(g, torch, T, K, W, dist, device):
     return sec, g.dg_get_launch_count() - n0
 
 
-def profile_kernels(g, T, reps, elems_per_global_step, Np, Nfp, rs, peak, peak_src, ncu_traffic=None):
+def profile_kernels(g, T, reps, elems_per_global_step, Np, Nfp, rs, peak, peak_src, traffic=None):
     """Separate pass with one event pair per launch: per-kernel average durations inside the step.
     achieved = algorithmic bytes of all launches of the class / their summed event time."""
     g.dg_step(min(T, 50))
@@ -214,11 +231,15 @@ def profile_kernels(g, T, reps, elems_per_global_step, Np, Nfp, rs, peak, peak_s
         ker[name] = {"launches": n, "avg_us": round(ms * 1e3 / n, 3),
                      "algorithmic_bytes_per_launch": int(nbytes / n),
                      "achieved_gbs": round(gbs, 1), "frac": round(gbs / peak, 4)}
+        tr = traffic(name) if traffic else None
+        ker[name]["traffic"] = tr              # ncu dram bytes per launch of this kernel on this workload, or null
+        if tr:
+            ker[name]["frac_dram"] = round(tr / (ms * 1e-3 / n) * 1e-9 / peak, 4)
     total = sum(v[0] for v in times.values())
     other = total - sum(times[k][0] for k in ker)
     dom = max(ker, key=lambda k: times[k][0])
     roof = {"bound": "hbm", "kernel": dom, "achieved": ker[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-            "frac": ker[dom]["frac"], "traffic": ncu_traffic, "peak_source": peak_src,
+            "frac": ker[dom]["frac"], "traffic": ker[dom]["traffic"], "peak_source": peak_src,
             "share_of_step": round(times[dom][0] / total, 4) if total else None}
     return roof, ker, {"other_kernels_ms": round(other, 3), "all_kernels_ms": round(total, 3)}
 
@@ -242,7 +263,20 @@ def run_e2e(g, torch, T, K, q0, device):
 # --------------------------------------------------------------------------------------------------
 # the oracle on the host cores: cpu_baseline and --impl reference
 # --------------------------------------------------------------------------------------------------
-def oracle_threads():
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def blas_threads():
+    """Size of the BLAS thread pool numpy would use (NOT the cores the oracle keeps busy: its element loops are
+    serial numpy; only the matrix products inside go to BLAS)."""
     try:
         from threadpoolctl import threadpool_info
         n = [p.get("num_threads", 1) for p in threadpool_info()]
@@ -267,18 +301,33 @@ def time_oracle(o, F, nglobal, t0):
     return time.perf_counter() - t
 
 
-def cpu_baseline(cfg, budget_s=15.0):
-    """The oracle as it stands on a bounded sample: as many global time steps of the same workload as
-    fit in about budget_s seconds (the rate does not depend on the step count)."""
+def cpu_baseline(cfg, budget_s=10.0):
+    """The oracle as it stands on a bounded sample: as many global time steps of the same workload as fit in about
+    budget_s seconds (the rate does not depend on the step count), timed twice as SURVEY.md 8(d) / BASELINE.md 3 ask:
+    with the BLAS pool at nproc threads and with 1 thread."""
+    from threadpoolctl import threadpool_limits
     o = make_oracle(cfg)
     F = o.new_field()
     dt_g = o.dt_local * o.nlocal
-    sec1 = time_oracle(o, F, 1, 0.0)
-    n = int(max(1, min(50, budget_s / max(sec1, 1e-3))))
-    sec = time_oracle(o, F, n, dt_g)
     dof = dof_updates_per_global_step(o.level, o.Np)
-    return {"value": dof * n / sec, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
-            "sample": "%d global time steps of %s (K=%d, N=%d, fp64 numpy), %.1f s" % (n, cfg["name"], o.K, cfg["N"], sec)}
+    nproc = os.cpu_count() or 1
+    runs = {}
+    done = 0
+    for label, nth in (("all", nproc), ("one", 1)):
+        with threadpool_limits(limits=nth):
+            sec1 = time_oracle(o, F, 1, done * dt_g)
+            done += 1
+            n = int(max(1, min(50, budget_s / max(sec1, 1e-3))))
+            sec = time_oracle(o, F, n, done * dt_g)
+            done += n
+        runs[label] = (dof * n / sec, n, sec)
+    v, n, sec = runs["all"]
+    return {"value": v, "unit": UNIT, "cores": nproc, "kind": "oracle",
+            "threads": "numpy fp64 oracle; element loops are serial numpy, only the matrix products use the BLAS pool "
+                       "(%d threads = nproc for `value`, 1 thread for `value_1_thread`)" % nproc,
+            "value_1_thread": runs["one"][0], "nproc": nproc, "cpu_model": cpu_model(),
+            "sample": "%d global time steps of %s (K=%d, N=%d, fp64 numpy), %.1f s; 1 thread: %d steps, %.1f s"
+                      % (n, cfg["name"], o.K, cfg["N"], sec, runs["one"][1], runs["one"][2])}
 
 
 def run_reference(args):
@@ -310,7 +359,9 @@ def run_reference(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg["name"], "K": int(o.K), "N": cfg["N"], "hexes": list(cfg["hexes"]),
                        "note": "the reference is a paper: this arm is the fp64 numpy oracle on the host cores"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle",
+                             "threads": "numpy fp64 oracle, BLAS pool %d threads, element loops serial" % blas_threads(),
+                             "cpu_model": cpu_model(), "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -319,7 +370,7 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------------
 # extras (rank 0, N = 1): the other items of BASELINE.json's metric
 # --------------------------------------------------------------------------------------------------
-def extra_sweep(torch, device, peak, peak_src, hexes):
+def extra_sweep(torch, device, peak, peak_src, hexes, traffic_table):
     """DOF-updates/s and per-kernel GB/s at N = 3, 4 in fp32 and fp64 on a mesh far larger than L2
     (config-4-sized jittered box, single-rate) and with the three LTS levels of config 3's grading."""
     from workloads import make_config
@@ -332,7 +383,8 @@ def extra_sweep(torch, device, peak, peak_src, hexes):
         levels = g.dg_get_levels()
         dof = dof_updates_per_global_step(levels, g.Np)
         sec, _ = timed_steps(g, torch, T, 3, 1, None, device)
-        roof, ker, oth = profile_kernels(g, T, 1, dof // (4 * g.Np), g.Np, g.Nfp, prec // 8, peak, peak_src)
+        roof, ker, oth = profile_kernels(g, T, 1, dof // (4 * g.Np), g.Np, g.Nfp, prec // 8, peak, peak_src,
+                                         traffic=lambda k, name=name, N=N, prec=prec: traffic_of(traffic_table, name, N, prec, k))
         out.append({"workload": name, "K": int(g.K), "N": N, "dtype": "f%d" % prec,
                     "levels": np.bincount(levels).tolist(), "value": dof * T * 3 / sec, "unit": UNIT,
                     "ms_per_global_time_step": 1e3 * sec / (3 * T), "kernels": ker, **oth})
@@ -340,6 +392,87 @@ def extra_sweep(torch, device, peak, peak_src, hexes):
         del g
         torch.cuda.empty_cache()
     return out
+
+
+def extra_cfg5_sweep(torch, device, peak, hexes, nglobal=5):
+    """BASELINE.json config 5: 96 x 96 x 48 hexahedra x 6 tetrahedra, orders 1..6, fp32 and fp64, three multi-rate levels:
+    DOF-updates/s and the fraction of the HBM roofline (algorithmic bytes of the fused step) per entry."""
+    from workloads import make_config
+    base = make_config("cfg5_sweep", hexes=hexes)
+    out = []
+    for prec in (32, 64):
+        for N in (1, 2, 3, 4, 5, 6):
+            cfg = dict(base, N=N, precision=prec, receivers=None)
+            g = make_ctx(cfg, device)
+            levels = g.dg_get_levels()
+            dof = dof_updates_per_global_step(levels, g.Np)
+            sec, launches = timed_steps(g, torch, nglobal, 2, 1, None, device)
+            nbytes = dof // (4 * g.Np) * algorithmic_scalars("step", g.Np, g.Nfp) * (prec // 8)     # per global step
+            gbs = nbytes * 2 * nglobal / sec * 1e-9
+            out.append({"N": N, "dtype": "f%d" % prec, "K": int(g.K), "levels": np.bincount(levels).tolist(),
+                        "global_steps_timed": 2 * nglobal, "value": dof * 2 * nglobal / sec, "unit": UNIT,
+                        "single_rate_equivalent": 4 * int(g.K) * g.Np * (1 << (cfg["nlevels"] - 1)) * 2 * nglobal / sec,
+                        "ms_per_global_time_step": 1e3 * sec / (2 * nglobal), "achieved_gbs": round(gbs, 1),
+                        "frac": round(gbs / peak, 4), "workspace_gb": round(g.dg_workspace_bytes() * 1e-9, 2)})
+            g.close()
+            del g
+            torch.cuda.empty_cache()
+    return out
+
+
+def extra_unfused_kernels(torch, device, peak, hexes, traffic_table):
+    """The paper's own kernel split (volume, surface, update; image kernel PAPER.md:204) as stand-alone
+    launches over the config-4 mesh through dg_bench_kernel, beside the fused step: per kernel the algorithmic bytes of
+    SURVEY.md 8(d)'s table / time against the HBM roofline (north_star: volume / surface / update kernels each)."""
+    from workloads import make_config
+    out = []
+    which = (("volume", 0, lambda Np, Nfp: 8 * Np + 11), ("surface", 1, lambda Np, Nfp: 8 * Np + 16 * Nfp + 20),
+             ("update", 3, lambda Np, Nfp: 20 * Np + 8 * Nfp),
+             ("update_two_fields_with_imaging", 4, lambda Np, Nfp: 2 * (20 * Np + 8 * Nfp) + 2 * Np))
+    for N, prec in ((3, 32), (4, 32), (3, 64), (4, 64)):
+        cfg = make_config("cfg4_rtm", hexes=hexes, N=N, precision=prec, nsteps=2, n_receivers_side=2)
+        g = make_ctx(cfg, device, history_steps=2)
+        rng = np.random.default_rng(1)
+        g.dg_set_state(1e-3 * rng.standard_normal((g.K, 4, g.Np)))
+        entry = {"workload": "cfg4_rtm", "K": int(g.K), "N": N, "dtype": "f%d" % prec, "kernels": {}}
+        for name, w, scal in which:
+            reps = 10
+            g.dg_bench_kernel(w, 3)
+            torch.cuda.synchronize(device)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            g.dg_bench_kernel(w, reps)
+            e1.record()
+            torch.cuda.synchronize(device)
+            us = e0.elapsed_time(e1) * 1e3 / reps
+            nbytes = int(g.K) * scal(g.Np, g.Nfp) * (prec // 8)
+            entry["kernels"][name] = {"avg_us": round(us, 2), "algorithmic_bytes_per_launch": nbytes,
+                                      "achieved_gbs": round(nbytes / us * 1e-3, 1), "frac": round(nbytes / us * 1e-3 / peak, 4),
+                                      "traffic": traffic_of(traffic_table, "cfg4_rtm", N, prec, name)}
+        out.append(entry)
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+    return out
+
+
+def measured_alu_peaks(device, peak_hbm):
+    """Register-only FMA ceilings (dg_measure_fma) and, per order, which roof bounds the fused step: the time the
+    method's flops (12 Np^2 + 32 Np Nfp per element) need at the FMA ceiling against the time its
+    algorithmic bytes need at the HBM ceiling."""
+    import paper_1506_00907_b200 as pk
+    f32, f32x2, f64 = (pk.dg_measure_fma(k, device) for k in (0, 1, 2))
+    binds = {}
+    for N in range(1, 7):
+        Np, Nfp = (N + 1) * (N + 2) * (N + 3) // 6, (N + 1) * (N + 2) // 2
+        flops = 12 * Np * Np + 32 * Np * Nfp
+        scal = algorithmic_scalars("step", Np, Nfp)
+        for tag, pk_tf, rs in (("f32", max(f32, f32x2), 4), ("f64", f64, 8)):
+            t_fma, t_hbm = flops / (pk_tf * 1e12), scal * rs / (peak_hbm * 1e9)
+            binds["N%d_%s" % (N, tag)] = {"fma_over_hbm_time": round(t_fma / t_hbm, 3), "bound": "alu" if t_fma > t_hbm else "hbm"}
+    return {"fp32_fma_tflops": round(f32, 2), "fp32_ffma2_tflops": round(f32x2, 2), "fp64_fma_tflops": round(f64, 2),
+            "how": "dg_measure_fma: 16 independent register chains per thread, 8 x 256 threads per SM, best of 3",
+            "fused_step_bound_by_order": binds}
 
 
 def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps):
@@ -382,6 +515,95 @@ def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps):
     return out
 
 
+def survey_shots(nshots, lengths, hexes, receivers):
+    """Seeded shot list of a survey over one mesh ("29 gathers"): sources along a line at the top, each
+    with its own receiver set (a shifted sub-grid, so the counts differ between gathers)."""
+    hx = lengths[0] / hexes[0]
+    hz = lengths[2] / hexes[2]
+    shots = []
+    for s in range(nshots):
+        fx = 0.2 + 0.6 * (s + 0.5) / nshots
+        x0 = np.array([fx * lengths[0] + 0.013 * hx, 0.5 * lengths[1] + 0.007 * hx, 0.25 * hz])
+        rcv = receivers[s % 3::3] + np.array([0.003 * (s % 5) * hx, 0.002 * (s % 7) * hx, 0.0])
+        shots.append(dict(index=s, x0=x0, receivers=rcv))
+    return shots
+
+
+def shots_of_rank(nshots, rank, world):
+    """Round-robin split of the shot indices over the ranks (shots are independent)."""
+    return list(range(rank, nshots, world))
+
+
+def stack_images(image, dist):
+    """The survey's one collective: the images of all replicas add.  `image` is a torch tensor (the
+    device view of the library's image, or a CPU tensor in the gloo test); summed in place on every rank."""
+    if dist is not None:
+        dist.all_reduce(image, op=dist.ReduceOp.SUM)
+    return image
+
+
+def run_survey(args, torch, dist, device, world, rank, peak):
+    from workloads import make_config
+    hexes = tuple(int(x) for x in args.hexes.split(",")) if args.hexes else None
+    cfg = make_config("cfg4_rtm", hexes=hexes, N=args.order or None, precision=args.precision or None,
+                      nsteps=args.timesteps or None)
+    nsteps = cfg["nsteps"]
+    nshots = max(1, args.steps) * world                     # weak scaling: `--steps` shots per GPU
+    shots = survey_shots(nshots, cfg["lengths"], cfg["hexes"], cfg["receivers"])
+    mine = shots_of_rank(nshots, rank, world)
+    t_setup = time.perf_counter()
+    g = make_ctx(dict(cfg, receivers=None), device)         # preparatory phase: once for the whole survey (PAPER.md:478)
+    g.rtm_set_receiver_capacity(max(len(sh["receivers"]) for sh in shots))
+    g.bind_history_torch(nsteps, device)
+    t_setup = time.perf_counter() - t_setup
+    src = cfg["source"]
+    updir = tuple(cfg["updir"])
+
+    def one_shot(sh):
+        g.dg_set_source(sh["x0"], src["f0"], src["tp"], src["amp"])
+        g.dg_set_receivers(sh["receivers"])
+        g.rtm_forward_shot(nsteps, want_data=False)
+        g.rtm_backward_shot(nsteps, None, updir=updir)     # the signals recorded on the device are re-injected
+
+    for _ in range(min(1, max(args.warmup, 0))):            # one untimed shot (the first launch of every kernel)
+        one_shot(shots[mine[0]])
+    g.rtm_image_zero()
+    torch.cuda.synchronize(device)
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    sampler.start()
+    n0 = g.dg_get_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for s in mine:
+        one_shot(shots[s])
+    img = stack_images(g.image_torch(), dist)
+    e1.record()
+    torch.cuda.synchronize(device)
+    if dist is not None:
+        dist.barrier()
+    sec = max_over_ranks(e0.elapsed_time(e1) * 1e-3, dist, device)
+    clocks = sampler.stop()
+    launches = g.dg_get_launch_count() - n0
+    image_l2 = float(np.linalg.norm(g.rtm_image_read()))
+    dof_shot = 4 * int(g.K) * g.Np * nsteps * 3             # forward + two wavefields backward
+    line = {"metric": METRIC, "value": dof_shot * nshots / sec, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sec / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f%d" % cfg["precision"], "data": "synthetic",
+            "config": {"workload": "survey", "mesh": "cfg4_rtm", "hexes": list(cfg["hexes"]), "K": int(g.K), "N": cfg["N"],
+                       "shots": nshots, "shots_per_gpu": len(mine), "time_steps_per_shot": "%d forward + %d backward" % (nsteps, nsteps),
+                       "receivers_per_shot": [int(len(sh["receivers"])) for sh in shots][:8],
+                       "parallelism": "shot per GPU x%d, one image all-reduce at the end" % world,
+                       "l2": "inputs far larger than L2 (1.9 GB per time step)"},
+            "shots_per_s": nshots / sec, "shot_s": sec / len(mine), "setup_s_once_per_survey": t_setup,
+            "image_bytes_allreduced": int(img.numel() * img.element_size()) if dist is not None else 0,
+            "image_l2": image_l2, "gpu_launches": int(launches), "clocks": clocks}
+    g.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
 def run_ours(args):
     import torch
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -398,6 +620,12 @@ def run_ours(args):
         dist_mod.init_process_group("nccl", device_id=torch.device(device))
         dist = dist_mod
     peak, peak_src = load_peaks()
+    traffic_table = load_traffic()
+    if args.workload == "survey":
+        run_survey(args, torch, dist, device, world, rank, peak)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     cfg, T = build_workload(args)
     g = make_ctx(cfg, device)
     levels = g.dg_get_levels()
@@ -413,7 +641,7 @@ def run_ours(args):
 
     # roofline of the dominant kernel: separate pass, one event pair per launch
     roof, ker, oth = profile_kernels(g, T, max(1, min(K, 3)), dof_step // (4 * Np), Np, Nfp, rs, peak, peak_src,
-                                     ncu_traffic=NCU_TRAFFIC.get((cfg["name"], cfg["N"], cfg["precision"])))
+                                     traffic=lambda k: traffic_of(traffic_table, cfg["name"], cfg["N"], cfg["precision"], k))
     roof["timing"] = "one CUDA event pair per launch (dg_set_profiling), separate pass over the same steps"
     if len(ker) == 1 and oth["other_kernels_ms"] == 0.0 and launches == K * T * (1 << (cfg["nlevels"] - 1)):
         # the step is ONE kernel launched back to back: its average launch duration over the timed region is
@@ -424,6 +652,8 @@ def run_ours(args):
         roof["event_pair_pass"] = {"avg_us": ker[dom]["avg_us"], "achieved": roof["achieved"], "frac": roof["frac"]}
         roof["achieved"] = round(nbytes / avg_s * 1e-9, 1)
         roof["frac"] = round(nbytes / avg_s * 1e-9 / peak, 4)
+        if roof["traffic"]:
+            roof["frac_dram"] = round(roof["traffic"] / avg_s * 1e-9 / peak, 4)
         roof["avg_launch_us"] = round(avg_s * 1e6, 3)
         roof["timing"] = "CUDA events around the timed region / launches in it (the step is this one kernel)"
 
@@ -455,19 +685,17 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_extras:
         line["cpu_baseline"] = cpu_baseline(cfg)
         big = args.workload == "cfg2_two_layer" and not args.hexes
+        line["peaks"] = measured_alu_peaks(device, peak)
         line["sweep_large_mesh"] = extra_sweep(torch, device, peak, peak_src,
-                                               {} if big else {"cfg4_rtm": (8, 8, 4), "cfg3_lts": (8, 8, 8)})
+                                               {} if big else {"cfg4_rtm": (8, 8, 4), "cfg3_lts": (8, 8, 8)}, traffic_table)
+        line["unfused_kernels"] = extra_unfused_kernels(torch, device, peak, None if big else (8, 8, 4), traffic_table)
+        line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8))
         line["rtm_shot"] = extra_rtm_shot(torch, device, peak, peak_src, None if big else (8, 8, 4),
                                           None if big else 20)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/), keyed by (workload, N, precision); None until captured
-NCU_TRAFFIC = {("cfg2_two_layer", 3, 32): 199077632}      # profiles/r1b_fused_pipeline.md (148.27 MB read + 50.81 MB written)
 
 
 if __name__ == "__main__":

@@ -193,6 +193,11 @@ int dg_get_kernel_times(dg_ctx* ctx, double* ms, int64_t* count);
  * 4 backward update with fused imaging (two wavefields). */
 int dg_bench_kernel(dg_ctx* ctx, int which, int reps);
 
+/* Plain-ALU ceilings of the device for the roofline (needs no ctx): a register-only fused-multiply-add
+ * loop, kind 0 = fp32 FFMA, 1 = packed fp32x2 FFMA2, 2 = fp64 DFMA; dscratch = at least 4 bytes x 2048 x (SM count)
+ * of device memory (never written in practice), timed with a CUDA event pair on the stream; *tflops = 2 flop per FMA. */
+int dg_measure_fma(int kind, void* dscratch, size_t scratch_bytes, void* cuda_stream, double* tflops);
+
 #ifdef __cplusplus
 }
 #endif

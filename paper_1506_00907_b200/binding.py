@@ -81,6 +81,7 @@ SIGNATURES = {
     "dg_set_profiling": (_i, [_vp, _i]),
     "dg_get_kernel_times": (_i, [_vp, _pd, _pi64]),
     "dg_bench_kernel": (_i, [_vp, _i, _i]),
+    "dg_measure_fma": (_i, [_i, _vp, _sz, _vp, _pd]),
 }
 for _name, (_res, _args) in SIGNATURES.items():
     _fn = getattr(_lib, _name)
@@ -360,6 +361,19 @@ class DG:
 
     def dg_bench_kernel(self, which, reps):
         self._ck(_lib.dg_bench_kernel(self._h, int(which), int(reps)))
+
+
+def dg_measure_fma(kind, device="cuda:0"):
+    """TFLOP/s of a register-only FMA loop (kind 0 fp32 FFMA, 1 packed FFMA2, 2 fp64 DFMA)."""
+    import torch
+    buf = torch.empty(4 * 2048 * 256, dtype=torch.uint8, device=device)
+    out = _d()
+    with torch.cuda.device(device):
+        rc = _lib.dg_measure_fma(int(kind), _vp(buf.data_ptr()), buf.numel(), _vp(torch.cuda.current_stream(device).cuda_stream),
+                                 C.byref(out))
+    if rc != DG_OK:
+        raise DGError(rc, "dg_measure_fma")
+    return out.value
 
 
 def dg_version():

@@ -19,6 +19,7 @@ LIB = os.path.join(HERE, "libdgrtm.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC = os.path.join(CUDA_HOME, "bin", "nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+CUDA_SOURCES = ["fma_bench.cu"]
 HOST_SOURCES = ["refelem.cpp", "mesh_setup.cpp", "api_core.cpp", "api_bind.cpp", "api_step.cpp",
                 "api_rtm.cpp", "api_get.cpp"]
 
@@ -53,6 +54,12 @@ def build(force=False, orders=(1, 2, 3, 4, 5, 6), verbose=False):
             jobs.append([NVCC, "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xptxas", "-v", "-DDG_ORDER=%d" % n,
                          *os.environ.get("DG_NVCC_FLAGS", "").split(),     # tuning sweeps (-DDG_F3_TO=.. etc.)
                          "-Xcompiler", "-fPIC", "-c", src, "-o", obj])
+    for name in CUDA_SOURCES:          # order-independent device code
+        src = os.path.join(CSRC, name)
+        obj = os.path.join(OBJ, name.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
+            jobs.append([NVCC, "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC", "-c", src, "-o", obj])
     missing = [n for n in range(1, 7) if n not in orders]
     stub = os.path.join(OBJ, "kernels_missing.cpp")
     if missing:   # partial builds (development): unresolved orders return no table

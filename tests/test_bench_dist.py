@@ -41,3 +41,45 @@ def test_dof_update_count_follows_the_levels():
     # 3 levels: K_l * 2^level * 4 Np
     levels = np.array([0] * 10 + [1] * 5 + [2] * 2)
     assert bench.dof_updates_per_global_step(levels, 20) == (10 * 1 + 5 * 2 + 2 * 4) * 4 * 20
+
+
+def _survey_worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    nshots = 5
+    mine = bench.shots_of_rank(nshots, rank, world)
+    # stand-in for the per-rank stacked image: shot s contributes (s + 1) at entry s and 1 everywhere
+    img = torch.zeros(8, dtype=torch.float64)
+    for s in mine:
+        img += 1.0
+        img[s] += s + 1
+    bench.stack_images(img, dist)
+    out[rank] = (mine, img.tolist())
+    dist.destroy_process_group()
+
+
+def test_survey_shot_split_and_image_sum_gloo():
+    """Shot-per-rank survey: every shot is done by exactly one rank and the one collective, the image
+    all-reduce, gives every rank the sum over ALL shots."""
+    world = 2
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_survey_worker, args=(world, 29543, out), nprocs=world, join=True)
+    shots = sorted(out[0][0] + out[1][0])
+    assert shots == [0, 1, 2, 3, 4] and not set(out[0][0]) & set(out[1][0])
+    want = [5.0 + (s + 1 if s < 5 else 0) for s in range(8)]
+    assert out[0][1] == want and out[1][1] == want
+
+
+def test_survey_shot_list_is_seeded_and_varied():
+    import numpy as np
+    import bench
+    rcv = np.stack(np.meshgrid(np.linspace(0.3, 2.7, 6), np.linspace(0.3, 2.7, 6), [0.01], indexing="ij"), -1).reshape(-1, 3)
+    a = bench.survey_shots(4, (3.0, 3.0, 1.5), (8, 8, 4), rcv)
+    b = bench.survey_shots(4, (3.0, 3.0, 1.5), (8, 8, 4), rcv)
+    assert all(np.array_equal(x["x0"], y["x0"]) and np.array_equal(x["receivers"], y["receivers"]) for x, y in zip(a, b))
+    assert len({tuple(x["x0"]) for x in a}) == 4
+    assert all(0 < x["x0"][0] < 3.0 for x in a) and all(len(x["receivers"]) == 12 for x in a)
+    assert bench.shots_of_rank(7, 1, 3) == [1, 4]
