@@ -12,15 +12,21 @@
 #pragma once
 #include "step_kernel.cuh"
 
+#ifndef DG_DBG_SKIP
+#define DG_DBG_SKIP 0
+#endif
 namespace dgrtm {
 
 // TO outputs per warp, NT warps per block, G groups per CTA, QS = stages of the q ring (2: fetched one item
 // ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
 // RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: read from global in the
 // update phase after an L2 prefetch (saves 8Np rows of shared memory per group: more groups per SM)
-template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0; };
+template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0, TP = 0; };
 // F2 = 1: the volume contraction of the one-field fp32 kernel uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the
 // FMA instructions for twice the accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 977 -> 1020 us)
+// TP = 1 (with RS = 0): the two older right-hand sides of the warp's own output nodes are loaded from L2 in chunks
+// during the lift loop and PARKED in tensor memory (tcgen05.st; lane = element, columns = values), from where the update
+// reads them back (tcgen05.ld): shared memory and the register file are full, the 256 KB of tensor memory are idle
 // UG = 1: velocities -> U.G once per block, in place in shared memory; 0: every warp forms U.G on the fly
 // (9 more FMAs per input node and warp, two shared-memory passes and one barrier fewer)
 #ifndef DG_PIPE_FFMA2
@@ -44,7 +50,7 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #ifndef DG_P3_UG
 #define DG_P3_UG 0
 #endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG, F2 = DG_PIPE_FFMA2; };
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG, F2 = DG_PIPE_FFMA2, TP = 0; };
 #ifndef DG_P4_TO
 #define DG_P4_TO 9
 #endif
@@ -60,17 +66,23 @@ template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; sta
 #ifndef DG_P4_UG
 #define DG_P4_UG 1
 #endif
+#ifndef DG_P4_TP
+#define DG_P4_TP 1
+#endif
 #ifndef DG_P4_QS
 #define DG_P4_QS 1
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0, TP = DG_P4_TP; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
 #define DG_D3_G 3
 #endif
+#ifndef DG_D3_TP
+#define DG_D3_TP 1
+#endif
 #ifndef DG_D3_OFF
-template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0, F2 = 0; };
+template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0, F2 = 0, TP = DG_D3_TP; };
 #endif
 
 template <typename real, int N> struct PipeSmem {
@@ -116,6 +128,56 @@ __device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&o
   }
 }
 
+
+// tensor memory as a parking lot for per-lane values (32x32b shape: thread i of the warp <-> lane base + i, NW
+// consecutive 32-bit columns per thread)
+template <int NW> __device__ __forceinline__ void tmem_st(unsigned taddr, const unsigned (&r)[NW]) {
+  static_assert(NW == 8 || NW == 16, "8 or 16 columns");
+  if constexpr (NW == 8)
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+  else
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+                 "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+                 "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+template <int NW> __device__ __forceinline__ void tmem_ld(unsigned taddr, unsigned (&r)[NW]) {
+  static_assert(NW == 8 || NW == 16, "8 or 16 columns");
+  if constexpr (NW == 8)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]),
+                 "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr) : "memory");
+  else
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                   "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// eight reals <-> 8 (float) or 16 (double) 32-bit words
+template <typename real> struct Words8;
+template <> struct Words8<float> {
+  static constexpr int NW = 8;
+  static __device__ __forceinline__ void pack(const float (&v)[8], unsigned (&r)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r[i] = __float_as_uint(v[i]);
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[8], float (&v)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+  }
+};
+template <> struct Words8<double> {
+  static constexpr int NW = 16;
+  static __device__ __forceinline__ void pack(const double (&v)[8], unsigned (&r)[16]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { r[2 * i] = (unsigned)__double2loint(v[i]); r[2 * i + 1] = (unsigned)__double2hiint(v[i]); }
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[16], double (&v)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
+  }
+};
+
 template <typename real, int N, bool DUAL>
 __global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
 k_pipe(const __grid_constant__ StepArgs a) {
@@ -148,6 +210,14 @@ k_pipe(const __grid_constant__ StepArgs a) {
   real* pen = TR + 4 * REC * 32;                                  // [2NF][32], later trace staging [4REC][32]
   unsigned long long* full = bars + 3 * g;                        // [0], [1]: q stages; [2]: r1, r2
   unsigned long long* tabbar = bars + 3 * G;
+  // tensor-memory parking: per warp 8 TO reals (h1, h2 of its TO nodes, 4 fields); warps of one lane quarter side by side
+  constexpr bool PARK = Cfg::TP && !RS;
+  constexpr int PW = Words8<real>::NW;                            // 32-bit columns per node
+  constexpr int PCOLS_NEED = (G * NT + 3) / 4 * TO * PW;
+  constexpr int PCOLS = PCOLS_NEED <= 32 ? 32 : (PCOLS_NEED <= 64 ? 64 : (PCOLS_NEED <= 128 ? 128 : (PCOLS_NEED <= 256 ? 256 : 512)));
+  static_assert(!PARK || PCOLS_NEED <= 512, "tensor memory has 512 columns");
+  constexpr int PCN = (TO + 3) / 4;                               // nodes per chunk: one chunk per face of the lift loop
+  unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 3 * G + 1);
 
   {  // operator tables + Fmask + permutation table: one blob, laid out on the host exactly as here
     if (tid == 0) {
@@ -157,8 +227,18 @@ k_pipe(const __grid_constant__ StepArgs a) {
       mbar_expect_tx(tabbar, (unsigned)SM::ops_bytes);
       bulk_g2s(smem_raw, a.ops2_D3Q, (unsigned)SM::ops_bytes, tabbar);
     }
+    if constexpr (PARK) {
+      if (wg == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(PCOLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
     __syncthreads();
+    if constexpr (PARK) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   }
+  // this warp's parking columns: lanes of quarter wg % 4, columns of its rank wg / 4 within the quarter
+  const unsigned tpark = PARK ? (*tmem_slot + ((unsigned)((wg & 3) * 32) << 16) + (unsigned)((wg >> 2) * TO * PW)) : 0u;
   const real* myD = sD + (size_t)w * Np * RL;
   const real* myL = sL + (size_t)w * NF * LL;
 
@@ -309,7 +389,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
       for (int k = 0; k < FPW; ++k) {
         const int f = w + k * NT;
-        if (f < 4) {
+        if (f < ((DG_DBG_SKIP & 4) ? 0 : 4)) {
           const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32],
                      nz = geo[(GEO_FACE + 5 * f + 2) * 32], gs = geo[(GEO_FACE + 5 * f + 3) * 32],
                      Zf = geo[(GEO_FACE + 5 * f + 4) * 32];
@@ -412,7 +492,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       for (int k = 0; k < RL / 2; ++k) { aG2[k] = make_float2(0.f, 0.f); aD2[k] = make_float2(0.f, 0.f); }
       constexpr int UM2 = 5;
 #pragma unroll UM2
-      for (int m = 0; m < Np; ++m) {
+      for (int m = 0; m < ((DG_DBG_SKIP & 1) ? 0 : Np); ++m) {
         const float p = Q[m * 32 + lane];
         const float vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
         float ur, us, ut;
@@ -451,7 +531,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #endif
       constexpr int UM = DG_PIPE_UNROLL_M;
 #pragma unroll UM
-      for (int m = 0; m < Np; ++m) {
+      for (int m = 0; m < ((DG_DBG_SKIP & 1) ? 0 : Np); ++m) {
         const real p = Q[m * 32 + lane];
         real ur, us, ut;
         if (INPLACE) {
@@ -477,9 +557,38 @@ k_pipe(const __grid_constant__ StepArgs a) {
       }
     }
     group_sync<NT>(g);                          // every warp has read Q: the update may overwrite its tile's nodes
-    // ---- surface (Alg. 3, second half)
+    // ---- surface (Alg. 3, second half); with PARK, chunk f of the older right-hand sides (h1, h2 of PCN of this
+    // warp's nodes, 4 fields) is in flight from L2 during the lift of face f and parked in tensor memory after it
+    const real* h1g = static_cast<const real*>(L.r1[fi]) + base + (size_t)n0 * 32;
+    const real* h2g = static_cast<const real*>(L.r2[fi]) + base + (size_t)n0 * 32;
+    real hc[PARK ? PCN : 1][8];
+    auto load_chunk = [&](int c) {
+#pragma unroll
+      for (int j = 0; j < PCN; ++j) {
+        const int nn = c * PCN + j;
+        if (nn < TO && (TO * NT == Np || n0 + nn < Np)) {
+#pragma unroll
+          for (int fld = 0; fld < 4; ++fld) {
+            hc[j][fld] = __ldg(h1g + (fld * Np + nn) * 32);
+            hc[j][4 + fld] = __ldg(h2g + (fld * Np + nn) * 32);
+          }
+        }
+      }
+    };
+    auto park_chunk = [&](int c) {
+#pragma unroll
+      for (int j = 0; j < PCN; ++j) {
+        const int nn = c * PCN + j;
+        if (nn < TO) {                                             // warp-uniform: tcgen05.st is .aligned
+          unsigned wd[PW];
+          Words8<real>::pack(hc[j], wd);
+          tmem_st<PW>(tpark + (unsigned)(nn * PW), wd);
+        }
+      }
+    };
+    if constexpr (PARK) load_chunk(0);
 #pragma unroll 1
-    for (int f = 0; f < 4; ++f) {
+    for (int f = 0; f < ((DG_DBG_SKIP & 2) ? 0 : 4); ++f) {
       real av[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
@@ -506,7 +615,12 @@ k_pipe(const __grid_constant__ StepArgs a) {
       const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
+      if constexpr (PARK) {
+        park_chunk(f);
+        if (f + 1 < 4) load_chunk(f + 1);
+      }
     }
+    if constexpr (PARK) tmem_wait_st();
 
     // ---- point terms (eq (15)), update (18), imaging (24); the new values replace the tile's nodes in Q
     const bool need_half = L.qf_half[fi] != nullptr && (a.blkflag[b] & 1);
@@ -529,50 +643,63 @@ k_pipe(const __grid_constant__ StepArgs a) {
       const real* R2t = RS ? R2 + n0 * 32 + lane : static_cast<const real*>(L.r2[fi]) + base + (size_t)n0 * 32;
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) {
-        if (FULL || n0 + nn < Np) {
-          real r0v[4] = {rp[nn], rx[nn], ry[nn], rz[nn]}, qo[4], h1[4], h2[4], v[4];
-          if (pi >= 0) r0v[0] += pts * ptv[n0 + nn];
-          qo[0] = Qt[nn * 32];
+        {
+          if (FULL || n0 + nn < Np) {
+            real h1[4], h2[4];
+            if constexpr (PARK) {                                    // parked in tensor memory during the lift loop
+              unsigned wd[PW];
+              real hv[8];
+              tmem_ld<PW>(tpark + (unsigned)(nn * PW), wd);
+              tmem_wait_ld();
+              Words8<real>::unpack(wd, hv);
 #pragma unroll
-          for (int fld = 1; fld < 4; ++fld) qo[fld] = INPLACE ? vold[fld - 1][nn] : Qt[(fld * Np + nn) * 32];
-#pragma unroll
-          for (int fld = 0; fld < 4; ++fld) { h1[fld] = R1t[(fld * Np + nn) * 32]; h2[fld] = R2t[(fld * Np + nn) * 32]; }
-#pragma unroll
-          for (int fld = 0; fld < 4; ++fld) {
-            v[fld] = qo[fld] + (c0 * r0v[fld] + c1 * h1[fld] + c2 * h2[fld]);
-            r0p[(fld * Np + nn) * 32] = r0v[fld];
-            qp[(fld * Np + nn) * 32] = v[fld];
-            Qt[(fld * Np + nn) * 32] = v[fld];
-          }
-          if (imaging) {
-            const real A0 = qo[0] + sgn * Z * (ex * qo[1] + ey * qo[2] + ez * qo[3]);
-            const real A1 = r0v[0] + sgn * Z * (ex * r0v[1] + ey * r0v[2] + ez * r0v[3]);
-            const real A2 = h1[0] + sgn * Z * (ex * h1[1] + ey * h1[2] + ez * h1[3]);
-            const real A3 = h2[0] + sgn * Z * (ex * h2[1] + ey * h2[2] + ez * h2[3]);
-            if (fi == 0) {
-              simg[0][nn] = A0; simg[1][nn] = A1; simg[2][nn] = A2; simg[3][nn] = A3;
+              for (int fld = 0; fld < 4; ++fld) { h1[fld] = hv[fld]; h2[fld] = hv[4 + fld]; }
             } else {
-              const real S0 = simg[0][nn];
-              const real rA[3] = {simg[1][nn], simg[2][nn], simg[3][nn]};
-              const real rB[3] = {A1, A2, A3};
-              real acc = S0 * A0;
 #pragma unroll
-              for (int k = 0; k < 3; ++k) {
-                acc += dts * (real)L.abar[k] * (S0 * rB[k] + A0 * rA[k]);
-#pragma unroll
-                for (int k2 = 0; k2 < 3; ++k2) acc += dts * dts * (real)L.C[3 * k + k2] * rA[k] * rB[k2];
-              }
-              if (a.trapezoid)                  // (21): mean of the integrand at the step ends; the new values are q + sum_s c_s r_s
-                acc = (real)0.5 * (S0 * A0 + (S0 + (c0 * rA[0] + c1 * rA[1] + c2 * rA[2])) * (A0 + (c0 * rB[0] + c1 * rB[1] + c2 * rB[2])));
-              imgp[nn * 32] = imgv[nn] + adts * acc;
+              for (int fld = 0; fld < 4; ++fld) { h1[fld] = R1t[(fld * Np + nn) * 32]; h2[fld] = R2t[(fld * Np + nn) * 32]; }
             }
-          }
-          // value at the half step (19) = new value + sum_s d_s r_s; kept for the second trace pass
-          if (need_half) {
+            real r0v[4] = {rp[nn], rx[nn], ry[nn], rz[nn]}, qo[4], v[4];
+            if (pi >= 0) r0v[0] += pts * ptv[n0 + nn];
+            qo[0] = Qt[nn * 32];
 #pragma unroll
-            for (int fld = 0; fld < 4; ++fld) v[fld] += d0 * r0v[fld] + d1 * h1[fld] + d2 * h2[fld];
+            for (int fld = 1; fld < 4; ++fld) qo[fld] = INPLACE ? vold[fld - 1][nn] : Qt[(fld * Np + nn) * 32];
+#pragma unroll
+            for (int fld = 0; fld < 4; ++fld) {
+              v[fld] = qo[fld] + (c0 * r0v[fld] + c1 * h1[fld] + c2 * h2[fld]);
+              r0p[(fld * Np + nn) * 32] = r0v[fld];
+              qp[(fld * Np + nn) * 32] = v[fld];
+              Qt[(fld * Np + nn) * 32] = v[fld];
+            }
+            if (imaging) {
+              const real A0 = qo[0] + sgn * Z * (ex * qo[1] + ey * qo[2] + ez * qo[3]);
+              const real A1 = r0v[0] + sgn * Z * (ex * r0v[1] + ey * r0v[2] + ez * r0v[3]);
+              const real A2 = h1[0] + sgn * Z * (ex * h1[1] + ey * h1[2] + ez * h1[3]);
+              const real A3 = h2[0] + sgn * Z * (ex * h2[1] + ey * h2[2] + ez * h2[3]);
+              if (fi == 0) {
+                simg[0][nn] = A0; simg[1][nn] = A1; simg[2][nn] = A2; simg[3][nn] = A3;
+              } else {
+                const real S0 = simg[0][nn];
+                const real rA[3] = {simg[1][nn], simg[2][nn], simg[3][nn]};
+                const real rB[3] = {A1, A2, A3};
+                real acc = S0 * A0;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                  acc += dts * (real)L.abar[k] * (S0 * rB[k] + A0 * rA[k]);
+#pragma unroll
+                  for (int k2 = 0; k2 < 3; ++k2) acc += dts * dts * (real)L.C[3 * k + k2] * rA[k] * rB[k2];
+                }
+                if (a.trapezoid)                  // (21): mean of the integrand at the step ends; the new values are q + sum_s c_s r_s
+                  acc = (real)0.5 * (S0 * A0 + (S0 + (c0 * rA[0] + c1 * rA[1] + c2 * rA[2])) * (A0 + (c0 * rB[0] + c1 * rB[1] + c2 * rB[2])));
+                imgp[nn * 32] = imgv[nn] + adts * acc;
+              }
+            }
+            // value at the half step (19) = new value + sum_s d_s r_s; kept for the second trace pass
+            if (need_half) {
+#pragma unroll
+              for (int fld = 0; fld < 4; ++fld) v[fld] += d0 * r0v[fld] + d1 * h1[fld] + d2 * h2[fld];
+            }
+            rp[nn] = v[0]; rx[nn] = v[1]; ry[nn] = v[2]; rz[nn] = v[3];
           }
-          rp[nn] = v[0]; rx[nn] = v[1]; ry[nn] = v[2]; rz[nn] = v[3];
         }
       }
     }
@@ -582,7 +709,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
     // per face from Q, placed at the reader's positions (permutation table), staged in pen as [row][lane]
 #pragma unroll 1
-    for (int pass = 0; pass < (need_half ? 2 : 1); ++pass) {
+    for (int pass = 0; pass < ((DG_DBG_SKIP & 8) ? 0 : (need_half ? 2 : 1)); ++pass) {
       if (pass == 1) {
         group_sync<NT>(g);                      // pass 0 has gathered from Q
         constexpr bool FULL = TO * NT == Np;
@@ -644,6 +771,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
     }
 #pragma unroll
     for (int k = 0; k < FPW; ++k) { codeA[k] = codeB[k]; codeB[k] = codeC[k]; }
+  }
+  if constexpr (PARK) {                         // every warp is done with its columns: release the tensor memory
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (wg == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "r"(PCOLS));
   }
 }
 
