@@ -32,6 +32,9 @@ template <typename real, int N> struct PipeCfg { static constexpr bool enabled =
 #ifndef DG_PIPE_FFMA2
 #define DG_PIPE_FFMA2 1
 #endif
+#ifndef DG_PIPE_FFMA2_DUAL
+#define DG_PIPE_FFMA2_DUAL 1
+#endif
 #ifndef DG_P3_TO
 #define DG_P3_TO 5
 #endif
@@ -129,55 +132,6 @@ __device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&o
 }
 
 
-// tensor memory as a parking lot for per-lane values (32x32b shape: thread i of the warp <-> lane base + i, NW
-// consecutive 32-bit columns per thread)
-template <int NW> __device__ __forceinline__ void tmem_st(unsigned taddr, const unsigned (&r)[NW]) {
-  static_assert(NW == 8 || NW == 16, "8 or 16 columns");
-  if constexpr (NW == 8)
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
-                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
-  else
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
-                 "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
-                 "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
-}
-template <int NW> __device__ __forceinline__ void tmem_ld(unsigned taddr, unsigned (&r)[NW]) {
-  static_assert(NW == 8 || NW == 16, "8 or 16 columns");
-  if constexpr (NW == 8)
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]),
-                 "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr) : "memory");
-  else
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
-                   "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// eight reals <-> 8 (float) or 16 (double) 32-bit words
-template <typename real> struct Words8;
-template <> struct Words8<float> {
-  static constexpr int NW = 8;
-  static __device__ __forceinline__ void pack(const float (&v)[8], unsigned (&r)[8]) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) r[i] = __float_as_uint(v[i]);
-  }
-  static __device__ __forceinline__ void unpack(const unsigned (&r)[8], float (&v)[8]) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-  }
-};
-template <> struct Words8<double> {
-  static constexpr int NW = 16;
-  static __device__ __forceinline__ void pack(const double (&v)[8], unsigned (&r)[16]) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { r[2 * i] = (unsigned)__double2loint(v[i]); r[2 * i + 1] = (unsigned)__double2hiint(v[i]); }
-  }
-  static __device__ __forceinline__ void unpack(const unsigned (&r)[16], double (&v)[8]) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
-  }
-};
-
 template <typename real, int N, bool DUAL>
 __global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
 k_pipe(const __grid_constant__ StepArgs a) {
@@ -212,10 +166,14 @@ k_pipe(const __grid_constant__ StepArgs a) {
   unsigned long long* tabbar = bars + 3 * G;
   // tensor-memory parking: per warp 8 TO reals (h1, h2 of its TO nodes, 4 fields); warps of one lane quarter side by side
   constexpr bool PARK = Cfg::TP && !RS;
+  constexpr bool IPARK = DUAL;                                    // imaging scalars of the source field wait in tensor memory
   constexpr int PW = Words8<real>::NW;                            // 32-bit columns per node
-  constexpr int PCOLS_NEED = (G * NT + 3) / 4 * TO * PW;
+  constexpr int IW = Words4<real>::NW;                            // 32-bit columns per node of the imaging scalars
+  constexpr int WCOLS = (PARK ? TO * PW : 0) + (IPARK ? TO * IW : 0);   // columns of one warp
+  constexpr int PCOLS_NEED = (G * NT + 3) / 4 * WCOLS;
   constexpr int PCOLS = PCOLS_NEED <= 32 ? 32 : (PCOLS_NEED <= 64 ? 64 : (PCOLS_NEED <= 128 ? 128 : (PCOLS_NEED <= 256 ? 256 : 512)));
-  static_assert(!PARK || PCOLS_NEED <= 512, "tensor memory has 512 columns");
+  static_assert(PCOLS_NEED <= 512, "tensor memory has 512 columns");
+  constexpr bool TMEM = PARK || IPARK;
   constexpr int PCN = (TO + 3) / 4;                               // nodes per chunk: one chunk per face of the lift loop
   unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 3 * G + 1);
 
@@ -227,7 +185,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       mbar_expect_tx(tabbar, (unsigned)SM::ops_bytes);
       bulk_g2s(smem_raw, a.ops2_D3Q, (unsigned)SM::ops_bytes, tabbar);
     }
-    if constexpr (PARK) {
+    if constexpr (TMEM) {
       if (wg == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(PCOLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
@@ -235,10 +193,11 @@ k_pipe(const __grid_constant__ StepArgs a) {
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();
-    if constexpr (PARK) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if constexpr (TMEM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   }
   // this warp's parking columns: lanes of quarter wg % 4, columns of its rank wg / 4 within the quarter
-  const unsigned tpark = PARK ? (*tmem_slot + ((unsigned)((wg & 3) * 32) << 16) + (unsigned)((wg >> 2) * TO * PW)) : 0u;
+  const unsigned tpark = TMEM ? (*tmem_slot + ((unsigned)((wg & 3) * 32) << 16) + (unsigned)((wg >> 2) * WCOLS)) : 0u;
+  const unsigned timg = tpark + (unsigned)(PARK ? TO * PW : 0);
   const real* myD = sD + (size_t)w * Np * RL;
   const real* myL = sL + (size_t)w * NF * LL;
 
@@ -354,7 +313,6 @@ k_pipe(const __grid_constant__ StepArgs a) {
   for (int k = 0; k < FPW; ++k)
 #pragma unroll
     for (int i2 = 0; i2 < Nfp; ++i2) fofs[k][i2] = (w + k * NT < 4 ? sF[(w + k * NT) * Nfp + i2] : 0) * 32 + lane;
-  real simg[4][TO];                                               // imaging scalars of the source field
 
 #pragma unroll 1
   for (int i = 0; i < nitems; ++i) {
@@ -367,7 +325,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     const real c0 = (real)L.c[0], c1 = (real)L.c[1], c2 = (real)L.c[2];
 
     group_sync<NT>(g);                          // the group has left the previous item (pen is free)
-    if (QS == 1 && i > 0) issue_q(i, 0);
+    if (QS == 1 && i > 0 && (DG_DBG_SKIP & 8)) issue_q(i, 0);
     mbar_wait(&full[s], (unsigned)(QS == 2 ? (i >> 1) : i) & 1u);
     cp_async_wait_all();
     __syncwarp();                               // the pieces of my record were fetched by other lanes of this warp
@@ -485,7 +443,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- volume (eqs (13)-(14), Alg. 2)
     real rp[TO], rx[TO], ry[TO], rz[TO];
-    if constexpr (sizeof(real) == 4 && !DUAL && Cfg::F2) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
+    if constexpr (sizeof(real) == 4 && Cfg::F2 && (!DUAL || DG_PIPE_FFMA2_DUAL)) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
                                                  // (the two-field kernel is register-bound and keeps scalar FMAs)
       float2 aG2[RL / 2], aD2[RL / 2];
 #pragma unroll
@@ -675,11 +633,21 @@ k_pipe(const __grid_constant__ StepArgs a) {
               const real A1 = r0v[0] + sgn * Z * (ex * r0v[1] + ey * r0v[2] + ez * r0v[3]);
               const real A2 = h1[0] + sgn * Z * (ex * h1[1] + ey * h1[2] + ez * h1[3]);
               const real A3 = h2[0] + sgn * Z * (ex * h2[1] + ey * h2[2] + ez * h2[3]);
-              if (fi == 0) {
-                simg[0][nn] = A0; simg[1][nn] = A1; simg[2][nn] = A2; simg[3][nn] = A3;
+              if (fi == 0) {                    // parked until the receiver field of this block is updated
+                const real sv[4] = {A0, A1, A2, A3};
+                unsigned wd[IW];
+                Words4<real>::pack(sv, wd);
+                tmem_st<IW>(timg + (unsigned)(nn * IW), wd);
               } else {
-                const real S0 = simg[0][nn];
-                const real rA[3] = {simg[1][nn], simg[2][nn], simg[3][nn]};
+                real sv[4];
+                {
+                  unsigned wd[IW];
+                  tmem_ld<IW>(timg + (unsigned)(nn * IW), wd);
+                  tmem_wait_ld();
+                  Words4<real>::unpack(wd, sv);
+                }
+                const real S0 = sv[0];
+                const real rA[3] = {sv[1], sv[2], sv[3]};
                 const real rB[3] = {A1, A2, A3};
                 real acc = S0 * A0;
 #pragma unroll
@@ -704,6 +672,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       }
     }
 
+    if constexpr (IPARK) { if (fi == 0) tmem_wait_st(); }
     group_sync<NT>(g);                          // Q holds the new values; r1, r2 are consumed
     if (i + 1 < nitems) issue_r(i + 1);
     // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
@@ -740,6 +709,8 @@ k_pipe(const __grid_constant__ StepArgs a) {
         }
       }
       group_sync<NT>(g);
+      // single-stage q ring: the last pass has gathered from Q, so the next item's q may land during the write-out
+      if (QS == 1 && pass == (need_half ? 1 : 0) && i + 1 < nitems) issue_q(i + 1, 0);
       {  // cooperative write-out: the block's 32 x 4 records are one contiguous run; consecutive lanes store
          // consecutive 16-byte pieces (piece P = element-lane P / NV, rows VS (P % NV) ..)
         constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
@@ -772,7 +743,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
     for (int k = 0; k < FPW; ++k) { codeA[k] = codeB[k]; codeB[k] = codeC[k]; }
   }
-  if constexpr (PARK) {                         // every warp is done with its columns: release the tensor memory
+  if constexpr (TMEM) {                         // every warp is done with its columns: release the tensor memory
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (wg == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "r"(PCOLS));

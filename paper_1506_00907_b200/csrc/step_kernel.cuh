@@ -21,25 +21,35 @@
 
 namespace dgrtm {
 
+#ifndef DG_STEP_PARK
+#define DG_STEP_PARK 1
+#endif
 template <typename real, int N> struct StepCfg;
-//                                            TO = outputs per warp, NT = warps per block, G = groups per CTA
-template <> struct StepCfg<float, 1> { static constexpr int TO = 4, NT = 1, G = 16; };
-template <> struct StepCfg<float, 2> { static constexpr int TO = 12, NT = 1, G = 12; };
+//                                            TO = outputs per warp, NT = warps per block, G = groups per CTA,
+//                                            PK = older right-hand sides parked in tensor memory (N = 5 fp32: the
+//                                            96-register budget of its 21 warps has no room for the chunk in flight)
+template <> struct StepCfg<float, 1> { static constexpr int TO = 4, NT = 1, G = 16, PK = 1; };
+template <> struct StepCfg<float, 2> { static constexpr int TO = 12, NT = 1, G = 12, PK = 1; };
 #ifndef DG_F3_TO
 #define DG_F3_TO 10
 #define DG_F3_NT 2
 #define DG_F3_G 10
 #endif
-template <> struct StepCfg<float, 3> { static constexpr int TO = DG_F3_TO, NT = DG_F3_NT, G = DG_F3_G; };
-template <> struct StepCfg<float, 4> { static constexpr int TO = 12, NT = 3, G = 5; };
-template <> struct StepCfg<float, 5> { static constexpr int TO = 8, NT = 7, G = 3; };
-template <> struct StepCfg<float, 6> { static constexpr int TO = 12, NT = 7, G = 2; };
-template <> struct StepCfg<double, 1> { static constexpr int TO = 4, NT = 1, G = 12; };
-template <> struct StepCfg<double, 2> { static constexpr int TO = 10, NT = 1, G = 8; };
-template <> struct StepCfg<double, 3> { static constexpr int TO = 10, NT = 2, G = 5; };
-template <> struct StepCfg<double, 4> { static constexpr int TO = 12, NT = 3, G = 2; };
-template <> struct StepCfg<double, 5> { static constexpr int TO = 8, NT = 7, G = 1; };
-template <> struct StepCfg<double, 6> { static constexpr int TO = 12, NT = 7, G = 1; };
+template <> struct StepCfg<float, 3> { static constexpr int TO = DG_F3_TO, NT = DG_F3_NT, G = DG_F3_G, PK = 1; };
+template <> struct StepCfg<float, 4> { static constexpr int TO = 12, NT = 3, G = 5, PK = 1; };
+template <> struct StepCfg<float, 5> { static constexpr int TO = 8, NT = 7, G = 3, PK = 0; };
+template <> struct StepCfg<float, 6> { static constexpr int TO = 12, NT = 7, G = 2, PK = 1; };
+template <> struct StepCfg<double, 1> { static constexpr int TO = 4, NT = 1, G = 12, PK = 1; };
+template <> struct StepCfg<double, 2> { static constexpr int TO = 10, NT = 1, G = 8, PK = 1; };
+template <> struct StepCfg<double, 3> { static constexpr int TO = 10, NT = 2, G = 5, PK = 1; };
+#ifndef DG_S4D_TO
+#define DG_S4D_TO 6
+#define DG_S4D_NT 6
+#define DG_S4D_G 2
+#endif
+template <> struct StepCfg<double, 4> { static constexpr int TO = DG_S4D_TO, NT = DG_S4D_NT, G = DG_S4D_G, PK = 1; };
+template <> struct StepCfg<double, 5> { static constexpr int TO = 8, NT = 7, G = 1, PK = 1; };
+template <> struct StepCfg<double, 6> { static constexpr int TO = 12, NT = 7, G = 1, PK = 1; };
 
 template <typename real, int N, bool DUAL> struct StepSmem {
   using O = Order<N>;
@@ -60,9 +70,9 @@ template <typename real, int N, bool DUAL> struct StepSmem {
       ops_reals * sizeof(real) + tab_ints * sizeof(int) + 128 + 128 + 1024 + group_bytes <= 227 * 1024;
   static constexpr size_t raw = (ops_in_smem ? ops_reals * sizeof(real) : 0) + tab_ints * sizeof(int);
   static constexpr size_t ops_bytes = (raw + 127) / 128 * 128;
-  static constexpr int Gfit = (int)((227 * 1024 - 1024 - 128 - ops_bytes) / group_bytes);
+  static constexpr int Gfit = (int)((227 * 1024 - 1024 - 256 - ops_bytes) / group_bytes);
   static constexpr int G = Gfit < 1 ? 1 : (Gfit < C::G ? Gfit : C::G);
-  static constexpr size_t bytes = ops_bytes + 128 + (size_t)G * group_bytes;   // + mbarriers
+  static constexpr size_t bytes = ops_bytes + 256 + (size_t)G * group_bytes;   // + mbarriers, tensor-memory slot
   static_assert(NPAD >= O::Np, "tiles must cover Np");
 };
 
@@ -132,6 +142,83 @@ __device__ __forceinline__ void load_record(const real* __restrict__ p, real (&o
   }
 }
 
+// tensor memory as a parking lot for per-lane values (32x32b shape: thread i of the warp <-> lane base + i, NW
+// consecutive 32-bit columns per thread)
+template <int NW> __device__ __forceinline__ void tmem_st(unsigned taddr, const unsigned (&r)[NW]) {
+  static_assert(NW == 4 || NW == 8 || NW == 16, "4, 8 or 16 columns");
+  if constexpr (NW == 4)
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+  else if constexpr (NW == 8)
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+  else
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+                 "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+                 "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+template <int NW> __device__ __forceinline__ void tmem_ld(unsigned taddr, unsigned (&r)[NW]) {
+  static_assert(NW == 4 || NW == 8 || NW == 16, "4, 8 or 16 columns");
+  if constexpr (NW == 4)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr) : "memory");
+  else if constexpr (NW == 8)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]),
+                 "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr) : "memory");
+  else
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                   "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// eight reals <-> 8 (float) or 16 (double) 32-bit words
+template <typename real> struct Words8;
+template <> struct Words8<float> {
+  static constexpr int NW = 8;
+  static __device__ __forceinline__ void pack(const float (&v)[8], unsigned (&r)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r[i] = __float_as_uint(v[i]);
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[8], float (&v)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+  }
+};
+template <> struct Words8<double> {
+  static constexpr int NW = 16;
+  static __device__ __forceinline__ void pack(const double (&v)[8], unsigned (&r)[16]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { r[2 * i] = (unsigned)__double2loint(v[i]); r[2 * i + 1] = (unsigned)__double2hiint(v[i]); }
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[16], double (&v)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
+  }
+};
+
+template <typename real> struct Words4;
+template <> struct Words4<float> {
+  static constexpr int NW = 4;
+  static __device__ __forceinline__ void pack(const float (&v)[4], unsigned (&r)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) r[i] = __float_as_uint(v[i]);
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[4], float (&v)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) v[i] = __uint_as_float(r[i]);
+  }
+};
+template <> struct Words4<double> {
+  static constexpr int NW = 8;
+  static __device__ __forceinline__ void pack(const double (&v)[4], unsigned (&r)[8]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { r[2 * i] = (unsigned)__double2loint(v[i]); r[2 * i + 1] = (unsigned)__double2hiint(v[i]); }
+  }
+  static __device__ __forceinline__ void unpack(const unsigned (&r)[8], double (&v)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
+  }
+};
+
 // ---- the kernel ---------------------------------------------------------------------------------------
 template <typename real, int N, bool DUAL>
 __global__ void __launch_bounds__(StepSmem<real, N, DUAL>::G * StepCfg<real, N>::NT * 32, 1)
@@ -153,7 +240,7 @@ k_step(const __grid_constant__ StepArgs a) {
   int* sInv = sF + NF;                                            // [Np][3]
   int* sP = sInv + 3 * Np;                                        // [kMaxPerm][Nfp]
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::ops_bytes);
-  real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + 128);
+  real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + 256);
 
   const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
   real* qs = gbase + (size_t)g * SM::group_reals;                 // [4Np][32]
@@ -161,6 +248,16 @@ k_step(const __grid_constant__ StepArgs a) {
   real* sgeo = pen + 2 * NF * 32;                                 // [DG_NGEO][32]
   real* simg = sgeo + DG_NGEO * 32;                               // DUAL: [4][Np][32] (or global scratch)
   int* snbr = reinterpret_cast<int*>(simg + (SM::img_in_smem ? 4 * Np * 32 : 0));   // [4][32]
+  // the two older right-hand sides of the warp's own output nodes are loaded from L2 in chunks during the lift loop
+  // and PARKED in tensor memory (lane = element, columns = values; idle otherwise), where the update finds them
+  // without a global-load latency: per warp 8 TO reals, warps of one lane quarter side by side
+  constexpr bool PARK = DG_STEP_PARK != 0 && Cfg::PK;
+  constexpr int PW = Words8<real>::NW;                            // 32-bit columns per node
+  constexpr int PCOLS_NEED = (G * NT + 3) / 4 * TO * PW;
+  constexpr int PCOLS = PCOLS_NEED <= 32 ? 32 : (PCOLS_NEED <= 64 ? 64 : (PCOLS_NEED <= 128 ? 128 : (PCOLS_NEED <= 256 ? 256 : 512)));
+  static_assert(PCOLS_NEED <= 512, "tensor memory has 512 columns");
+  constexpr int PCN = (TO + 3) / 4;                               // nodes per chunk: one chunk per face of the lift loop
+  unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + G);
   constexpr unsigned GBYTES = DG_NGEO * 32 * sizeof(real), NBYTES = 4 * 32 * sizeof(int);
 
   {
@@ -173,8 +270,17 @@ k_step(const __grid_constant__ StepArgs a) {
     for (int i = tid; i < NF; i += NTHREADS) sF[i] = a.ops.Fmask[i];
     if (w == 0 && lane == 0) mbar_init(&bars[g], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if constexpr (PARK) {
+      if (wg == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(PCOLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
     load_face_tables<N>(a.ops, sInv, sP, NTHREADS);               // ends with __syncthreads
+    if constexpr (PARK) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   }
+  const unsigned tpark = PARK ? *tmem_slot + ((unsigned)((wg & 3) * 32) << 16) + (unsigned)((wg >> 2) * TO * PW) : 0u;
 
   const real* sD = OPS_SMEM ? sDs : static_cast<const real*>(a.ops.D3T);
   const real* sL = OPS_SMEM ? sLs : static_cast<const real*>(a.ops.LIFTT);
@@ -317,7 +423,36 @@ k_step(const __grid_constant__ StepArgs a) {
           rz[nn] = -irho * (g20 * aR[nn] + g21 * aS[nn] + g22 * aT[nn]);
         }
       }
-      // ---- surface (Alg. 3, second half): lift of the penalties; P^{v_i} = n_i * (scalar) per face
+      // ---- surface (Alg. 3, second half): lift of the penalties; P^{v_i} = n_i * (scalar) per face.  Chunk f of the
+      // older right-hand sides is in flight from L2 during the lift of face f and parked in tensor memory after it
+      const real* h1g = static_cast<const real*>(L.r1[fi]) + base + (size_t)n0 * 32;
+      const real* h2g = static_cast<const real*>(L.r2[fi]) + base + (size_t)n0 * 32;
+      real hc[PARK ? PCN : 1][8];
+      auto load_chunk = [&](int c) {
+#pragma unroll
+        for (int j = 0; j < PCN; ++j) {
+          const int nn = c * PCN + j;
+          if (nn < TO && n0 + nn < Np) {
+#pragma unroll
+            for (int fld = 0; fld < 4; ++fld) {
+              hc[j][fld] = __ldg(h1g + (fld * Np + nn) * 32);
+              hc[j][4 + fld] = __ldg(h2g + (fld * Np + nn) * 32);
+            }
+          }
+        }
+      };
+      auto park_chunk = [&](int c) {
+#pragma unroll
+        for (int j = 0; j < PCN; ++j) {
+          const int nn = c * PCN + j;
+          if (nn < TO) {                                           // warp-uniform: tcgen05.st is .aligned
+            unsigned wd[PW];
+            Words8<real>::pack(hc[j], wd);
+            tmem_st<PW>(tpark + (unsigned)(nn * PW), wd);
+          }
+        }
+      };
+      if constexpr (PARK) load_chunk(0);
 #pragma unroll 1
       for (int f = 0; f < 4; ++f) {
         real av[TO];
@@ -336,7 +471,12 @@ k_step(const __grid_constant__ StepArgs a) {
                    nz = geo[(GEO_FACE + 5 * f + 2) * 32];
 #pragma unroll
         for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
+        if constexpr (PARK) {
+          park_chunk(f);
+          if (f + 1 < 4) load_chunk(f + 1);
+        }
       }
+      if constexpr (PARK) tmem_wait_st();
 
       // ---- point terms (eq (15)), update (18), imaging (24); new values stay in rp/rx/ry/rz
       {
@@ -358,11 +498,20 @@ k_step(const __grid_constant__ StepArgs a) {
           if (n < Np) {
             real r0v[4] = {rp[nn], rx[nn], ry[nn], rz[nn]}, qo[4], h1[4], h2[4], v[4];
             if (pi >= 0) r0v[0] += pts * ptv[n];
+            if constexpr (PARK) {
+              unsigned wd[PW];
+              real hv[8];
+              tmem_ld<PW>(tpark + (unsigned)(nn * PW), wd);
+              tmem_wait_ld();
+              Words8<real>::unpack(wd, hv);
+#pragma unroll
+              for (int fld = 0; fld < 4; ++fld) { h1[fld] = hv[fld]; h2[fld] = hv[4 + fld]; }
+            }
 #pragma unroll
             for (int fld = 0; fld < 4; ++fld) {
               const size_t o = base + (size_t)(fld * Np + n) * 32;
               qo[fld] = (INPLACE && fld > 0) ? qg[o] : qs[(fld * Np + n) * 32 + lane];
-              h1[fld] = r1g[o]; h2[fld] = r2g[o];
+              if constexpr (!PARK) { h1[fld] = r1g[o]; h2[fld] = r2g[o]; }
             }
 #pragma unroll
             for (int fld = 0; fld < 4; ++fld) {
@@ -464,6 +613,11 @@ k_step(const __grid_constant__ StepArgs a) {
         }
       }
     }
+  }
+  if constexpr (PARK) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();                              // every warp is done with its columns: release the tensor memory
+    if (wg == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "r"(PCOLS));
   }
 }
 
