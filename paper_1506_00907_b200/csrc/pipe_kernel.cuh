@@ -67,15 +67,18 @@ template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; sta
 #define DG_P4_RS 0
 #endif
 #ifndef DG_P4_UG
-#define DG_P4_UG 1
+#define DG_P4_UG 0
 #endif
 #ifndef DG_P4_TP
 #define DG_P4_TP 1
 #endif
+#ifndef DG_P4_F2
+#define DG_P4_F2 0
+#endif
 #ifndef DG_P4_QS
 #define DG_P4_QS 1
 #endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = 0, TP = DG_P4_TP; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = DG_P4_F2, TP = DG_P4_TP; };
 #ifndef DG_D3_TO
 #define DG_D3_TO 5
 #define DG_D3_NT 4
