@@ -164,10 +164,11 @@ void upload_tables(dg_ctx* c) {
     upload_raw(c, c->d_stored[l], sf.data(), sf.size() * 4);
   }
   if (c->has_src) upload_real(c, c->d_src_w, c->src_w.data(), Np);
-  std::vector<unsigned char> flag((size_t)md.nblocks, 0);
+  std::vector<unsigned char> flag((size_t)md.nblocks + 32, 0);   // block flags, then the zeroed ticket counters
   for (int l = 0; l < md.nlevels; ++l)
     for (int32_t s : md.coarse_nb[l]) flag[s >> 5] |= 1;
   upload_raw(c, c->d_blkflag, flag.data(), flag.size());
+  c->sched_sel = 0;
   upload_point_source(c);
 }
 

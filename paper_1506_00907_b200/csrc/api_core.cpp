@@ -397,7 +397,7 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
     c->d_D3Q = cv.take(std::max<size_t>(16, c->kt ? c->kt->pipe_blob_bytes : 0));
     c->d_LTQ = cv.take(std::max<size_t>(16, c->kt ? c->kt->tc_blob_bytes : 0));      // tensor-core kernel's tables
   }
-  c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks);
+  c->d_blkflag = (unsigned char*)cv.take((size_t)md.nblocks + 32);   // + the ticket counters (sched_counters)
   c->d_pt_src = (int*)cv.take((size_t)md.nslots * 4);
   c->scratch = cv.take(field_bytes(c));
   c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);

@@ -78,6 +78,8 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.nfields = o.nfields; a.nlevels = L;
   a.geo = c->geo; a.nbr = c->nbr; a.wperm = c->wperm; a.blkflag = c->d_blkflag;
   a.ext = c->has_ext ? c->ext : nullptr;
+  a.sched = sched_counters(c);
+  a.sched_mode = L > 1 ? 1 : 0;     // blocks of a multi-rate launch differ in cost and sit sorted by level
   a.dir = (double)dir;
   a.ops = c->ops; a.ops.D3T = c->d_D3P; a.ops.LIFTT = c->d_LTP;
   a.ops2_D3Q = c->d_D3Q; a.ops2_LTQ = c->d_LTQ;
@@ -139,6 +141,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     a.blk0 = md.lvl_blk0[lmin];
     a.nblk = (int)md.nblocks - a.blk0;
     if (a.nblk > 0) {
+      if (pipe && (o.nfields == 2 || !tc)) { a.sched_sel = c->sched_sel; c->sched_sel ^= 1; }   // only launches that take tickets flip the counters
       if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, pipe ? c->kt->pipe2(a, c->stream) : c->kt->step2(a, c->stream));
       else DG_LAUNCH(c, KC_STEP, tc ? c->kt->tc(a, c->stream) : (pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream)));
     }

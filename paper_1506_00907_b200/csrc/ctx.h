@@ -129,7 +129,8 @@ struct dg_ctx {
   char* d_LTQ = nullptr;
   bool use_pipe = true;                     // DGRTM_KERNEL=step selects the non-pipelined fused kernel
   bool use_tc = false;                      // DGRTM_KERNEL=tc selects the tensor-core kernel (fp32, one wavefield)
-  unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour
+  unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour; then the ticket counters
+  int sched_sel = 0;                        // ticket counter the next pipelined launch uses (the kernel zeroes the other one)
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
@@ -168,6 +169,10 @@ namespace dgrtm {
 
 // ---- helpers shared by the api_*.cpp files
 size_t field_bytes(const dg_ctx* c);        // one [nslots][4Np] array
+// the two ticket counters of the pipelined kernel: 16-byte aligned behind the block flags (zeroed with them)
+inline unsigned* sched_counters(const dg_ctx* c) {
+  return reinterpret_cast<unsigned*>(((uintptr_t)c->d_blkflag + (size_t)c->model.nblocks + 15) & ~(uintptr_t)15);
+}
 size_t trace_bytes(const dg_ctx* c);        // one qf array
 void upload_real(dg_ctx* c, void* dst, const double* src, size_t n);
 void download_real(dg_ctx* c, double* dst, const void* src, size_t n);

@@ -121,6 +121,8 @@ struct StepArgs {
   int nlevels;
   const void* geo; const int* nbr; const int* wperm;
   const unsigned char* blkflag;   // per block: bit 0 = some element has a finer face neighbour
+  unsigned* sched; int sched_sel;   // two ticket counters of the pipelined kernel's work distribution; this launch uses [sched_sel]
+  int sched_mode;                   // 0: fixed contiguous chunks per CTA; 1: interleaved start, then blocks by ticket
   const void* ext;           // prescribed exterior states or null
   double dir;
   // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale

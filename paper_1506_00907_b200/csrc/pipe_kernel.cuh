@@ -204,21 +204,33 @@ k_pipe(const __grid_constant__ StepArgs a) {
   const real* myD = sD + (size_t)w * Np * RL;
   const real* myL = sL + (size_t)w * NF * LL;
 
+  // work distribution.  A group's j-th turn takes block base0 + j * stride while that is below `limit`, then blocks by
+  // ticket from a global counter (one atomic per block, taken three turns ahead).  sched_mode 0 (single-rate launches):
+  // fixed contiguous chunks per CTA, no tickets - the streams stay sequential and every block costs the same.
+  // sched_mode 1 (multi-rate launches): the first three turns interleaved over all groups, the rest by ticket - blocks
+  // differ in cost (levels, half-step traces) and sit sorted by level, so fixed chunks would load the SMs unevenly, and
+  // a launch of a few hundred blocks spreads over all SMs.  ring[j & 3] = block of the group's j-th turn, bend = none
+  int* ring = reinterpret_cast<int*>(smem_raw + SM::ops_bytes + 96) + 4 * g;
+  const int bend = a.blk0 + a.nblk, ngroups = (int)gridDim.x * G;
   const int lo = a.blk0 + (int)(((long long)a.nblk * blockIdx.x) / gridDim.x);
   const int hi = a.blk0 + (int)(((long long)a.nblk * (blockIdx.x + 1)) / gridDim.x);
-  const int nmine = (hi - lo - g + G - 1) / G;                    // blocks of this group
-  const int nitems = nmine > 0 ? nmine * NFLD : 0;
+  const bool tickets = a.sched_mode != 0;
+  const int base0 = tickets ? a.blk0 + g * (int)gridDim.x + (int)blockIdx.x : lo + g;
+  const int stride = tickets ? ngroups : G;
+  const long long dyn0 = (long long)a.blk0 + 3LL * ngroups;
+  const int limit = tickets ? (dyn0 < bend ? (int)dyn0 : bend) : hi;
+  unsigned* const ticket = a.sched + a.sched_sel;
   const real dir = (real)a.dir;
   const int n0 = w * TO;
 
-  auto item_block = [&](int i) { return lo + g + (i / NFLD) * G; };
+  auto item_block = [&](int i) { return ring[(i / NFLD) & 3]; };
   auto level_of = [&](int b) { int l = 0; while (b >= a.lv[l].blk_end) ++l; return l; };
   auto load_codes = [&](int i, int (&code)[FPW]) {
     const int b = item_block(i);
 #pragma unroll
     for (int k = 0; k < FPW; ++k) {
       const int f = w + k * NT;
-      code[k] = (f < 4 && i < nitems) ? a.nbr[((size_t)b * 4 + f) * 32 + lane] : -1;
+      code[k] = (f < 4 && b < bend) ? a.nbr[((size_t)b * 4 + f) * 32 + lane] : -1;
     }
   };
   // everything item i needs, into stage s: bulk copies by one lane, trace records by their consumer lanes
@@ -307,8 +319,14 @@ k_pipe(const __grid_constant__ StepArgs a) {
   // stream; from here on its results (q, right-hand sides, traces) are read
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (blockIdx.x == 0 && tid == 0) a.sched[a.sched_sel ^ 1] = 0u;   // the next launch's counter (this launch's predecessor is done with it)
+  if (w == 0 && lane < 3) {                     // the first three turns
+    const int bs = base0 + lane * stride;
+    ring[lane] = bs < limit ? bs : bend;        // (with tickets the first three turns are always the fixed ones)
+  }
+  group_sync<NT>(g);
   load_codes(0, codeA);
-  if (nitems > 0) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
+  if (item_block(0) < bend) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
   int fofs[FPW][Nfp];                                             // own-trace offsets of this warp's faces in Q
@@ -317,9 +335,13 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
     for (int i2 = 0; i2 < Nfp; ++i2) fofs[k][i2] = (w + k * NT < 4 ? sF[(w + k * NT) * Nfp + i2] : 0) * 32 + lane;
 
+  unsigned tk = 0;
 #pragma unroll 1
-  for (int i = 0; i < nitems; ++i) {
+  for (int i = 0; item_block(i) < bend; ++i) {
     const int s = QS == 2 ? (i & 1) : 0, b = item_block(i), fi = i % NFLD, l = level_of(b);
+    const bool more = item_block(i + 1) < bend;                   // another item follows
+    // ticket of the block three turns ahead: taken now, stored at the end of this block's last item
+    if (tickets && w == 0 && lane == 0 && fi == 0) tk = atomicAdd(ticket, 1u);
     const StepLevel& L = a.lv[l];
     real* Q = grp + (size_t)s * SM::stage_reals;                  // [4Np][32]
     const real* geo = Q + 4 * Np * 32 + lane;
@@ -421,7 +443,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
                g12 = geo[5 * 32], g20 = geo[6 * 32], g21 = geo[7 * 32], g22 = geo[8 * 32];
     group_sync<NT>(g);                          // penalties done; every warp has left the previous item
     // ---- the other stage is free now: fetch the next item; codes two items ahead
-    if (i + 1 < nitems) {
+    if (more) {
       if (QS == 2) issue_q(i + 1, s ^ 1); else prefetch_q(i + 1);
       issue_tr(i + 1, codeB);
     }
@@ -677,7 +699,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     if constexpr (IPARK) { if (fi == 0) tmem_wait_st(); }
     group_sync<NT>(g);                          // Q holds the new values; r1, r2 are consumed
-    if (i + 1 < nitems) issue_r(i + 1);
+    if (more) issue_r(i + 1);
     // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
     // per face from Q, placed at the reader's positions (permutation table), staged in pen as [row][lane]
 #pragma unroll 1
@@ -713,7 +735,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       }
       group_sync<NT>(g);
       // single-stage q ring: the last pass has gathered from Q, so the next item's q may land during the write-out
-      if (QS == 1 && pass == (need_half ? 1 : 0) && i + 1 < nitems) issue_q(i + 1, 0);
+      if (QS == 1 && pass == (need_half ? 1 : 0) && more) issue_q(i + 1, 0);
       {  // cooperative write-out: the block's 32 x 4 records are one contiguous run; consecutive lanes store
          // consecutive 16-byte pieces (piece P = element-lane P / NV, rows VS (P % NV) ..)
         constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
@@ -745,6 +767,10 @@ k_pipe(const __grid_constant__ StepArgs a) {
     }
 #pragma unroll
     for (int k = 0; k < FPW; ++k) { codeA[k] = codeB[k]; codeB[k] = codeC[k]; }
+    if (w == 0 && lane == 0 && fi == NFLD - 1) {                  // slot of the finished turn <- block three turns ahead
+      const long long bs = (long long)base0 + (long long)(i / NFLD + 3) * stride, nb = dyn0 + (long long)tk;
+      ring[(i / NFLD + 3) & 3] = tickets ? (nb < bend ? (int)nb : bend) : (bs < limit ? (int)bs : bend);
+    }
   }
   if constexpr (TMEM) {                         // every warp is done with its columns: release the tensor memory
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
