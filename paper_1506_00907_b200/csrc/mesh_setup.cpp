@@ -210,10 +210,21 @@ void build_model(const RefElem& re, const Mesh& m, const double* rho, const doub
   }
   md.nblocks = blk; md.nslots = (int64_t)blk * 32;
   md.slot_of.resize(K); md.elem_of.assign(md.nslots, -1);
-  for (int64_t k = 0; k < K; ++k) {
-    const int64_t s = next[md.level[k]]++;
-    md.slot_of[k] = s; md.elem_of[s] = k;
-  }
+  // within a level: first the elements with a finer face neighbour (they expose half-step traces, eq (19)), then
+  // the others, each in ascending element order - the blocks that need the second trace pass are as few as possible
+  auto has_finer = [&](int64_t k) {
+    for (int f = 0; f < 4; ++f) {
+      const int64_t k2 = m.EToE[4 * k + f];
+      if (k2 >= 0 && md.level[k2] > md.level[k]) return true;
+    }
+    return false;
+  };
+  for (int pass = 0; pass < 2; ++pass)
+    for (int64_t k = 0; k < K; ++k) {
+      if (has_finer(k) != (pass == 0)) continue;
+      const int64_t s = next[md.level[k]]++;
+      md.slot_of[k] = s; md.elem_of[s] = k;
+    }
   // ---- elements with a finer neighbour (coarse neighbours of Alg. 1)
   md.coarse_nb.assign(L, {});
   for (int l = 0; l < L; ++l)
