@@ -12,9 +12,6 @@
 #pragma once
 #include "step_kernel.cuh"
 
-#ifndef DG_DBG_SKIP
-#define DG_DBG_SKIP 0
-#endif
 namespace dgrtm {
 
 // TO outputs per warp, NT warps per block, G groups per CTA, QS = stages of the q ring (2: fetched one item
@@ -350,7 +347,6 @@ k_pipe(const __grid_constant__ StepArgs a) {
     const real c0 = (real)L.c[0], c1 = (real)L.c[1], c2 = (real)L.c[2];
 
     group_sync<NT>(g);                          // the group has left the previous item (pen is free)
-    if (QS == 1 && i > 0 && (DG_DBG_SKIP & 8)) issue_q(i, 0);
     mbar_wait(&full[s], (unsigned)(QS == 2 ? (i >> 1) : i) & 1u);
     cp_async_wait_all();
     __syncwarp();                               // the pieces of my record were fetched by other lanes of this warp
@@ -372,7 +368,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
       for (int k = 0; k < FPW; ++k) {
         const int f = w + k * NT;
-        if (f < ((DG_DBG_SKIP & 4) ? 0 : 4)) {
+        if (f < 4) {
           const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32],
                      nz = geo[(GEO_FACE + 5 * f + 2) * 32], gs = geo[(GEO_FACE + 5 * f + 3) * 32],
                      Zf = geo[(GEO_FACE + 5 * f + 4) * 32];
@@ -475,7 +471,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       for (int k = 0; k < RL / 2; ++k) { aG2[k] = make_float2(0.f, 0.f); aD2[k] = make_float2(0.f, 0.f); }
       constexpr int UM2 = 5;
 #pragma unroll UM2
-      for (int m = 0; m < ((DG_DBG_SKIP & 1) ? 0 : Np); ++m) {
+      for (int m = 0; m < Np; ++m) {
         const float p = Q[m * 32 + lane];
         const float vx = Q[(Np + m) * 32 + lane], vy = Q[(2 * Np + m) * 32 + lane], vz = Q[(3 * Np + m) * 32 + lane];
         float ur, us, ut;
@@ -514,7 +510,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #endif
       constexpr int UM = DG_PIPE_UNROLL_M;
 #pragma unroll UM
-      for (int m = 0; m < ((DG_DBG_SKIP & 1) ? 0 : Np); ++m) {
+      for (int m = 0; m < Np; ++m) {
         const real p = Q[m * 32 + lane];
         real ur, us, ut;
         if (INPLACE) {
@@ -571,7 +567,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     };
     if constexpr (PARK) load_chunk(0);
 #pragma unroll 1
-    for (int f = 0; f < ((DG_DBG_SKIP & 2) ? 0 : 4); ++f) {
+    for (int f = 0; f < 4; ++f) {
       real av[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
@@ -703,7 +699,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
     // ---- exposed traces (Alg. 4) of the new values, then of the half-step values (19): gathered
     // per face from Q, placed at the reader's positions (permutation table), staged in pen as [row][lane]
 #pragma unroll 1
-    for (int pass = 0; pass < ((DG_DBG_SKIP & 8) ? 0 : (need_half ? 2 : 1)); ++pass) {
+    for (int pass = 0; pass < (need_half ? 2 : 1); ++pass) {
       if (pass == 1) {
         group_sync<NT>(g);                      // pass 0 has gathered from Q
         constexpr bool FULL = TO * NT == Np;
