@@ -312,18 +312,16 @@ k_pipe(const __grid_constant__ StepArgs a) {
   };
 
   int codeA[FPW], codeB[FPW], codeC[FPW];
-  // programmatic dependent launch: everything above overlapped the tail of the previous launch on the
-  // stream; from here on its results (q, right-hand sides, traces) are read
+  // programmatic dependent launch: everything down to griddepcontrol.wait overlaps the tail of the previous launch
+  // on the stream and touches only what no launch writes (tables, neighbour codes); after it the previous launch's
+  // results (q, right-hand sides, traces, ticket counter) are read
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (blockIdx.x == 0 && tid == 0) a.sched[a.sched_sel ^ 1] = 0u;   // the next launch's counter (this launch's predecessor is done with it)
   if (w == 0 && lane < 3) {                     // the first three turns
     const int bs = base0 + lane * stride;
     ring[lane] = bs < limit ? bs : bend;        // (with tickets the first three turns are always the fixed ones)
   }
   group_sync<NT>(g);
   load_codes(0, codeA);
-  if (item_block(0) < bend) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
   int fofs[FPW][Nfp];                                             // own-trace offsets of this warp's faces in Q
@@ -331,6 +329,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
   for (int k = 0; k < FPW; ++k)
 #pragma unroll
     for (int i2 = 0; i2 < Nfp; ++i2) fofs[k][i2] = (w + k * NT < 4 ? sF[(w + k * NT) * Nfp + i2] : 0) * 32 + lane;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (blockIdx.x == 0 && tid == 0) a.sched[a.sched_sel ^ 1] = 0u;   // the next launch's counter (this launch's predecessor is done with it)
+  if (item_block(0) < bend) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
 
   unsigned tk = 0;
 #pragma unroll 1
