@@ -68,9 +68,14 @@ template <typename real> struct Launch {
                              (int)StepSmem<real, N, true>::bytes);
     if (e != cudaSuccess) return (int)e;
     if constexpr (PipeCfg<real, N>::enabled) {
-      e = cudaFuncSetAttribute(k_pipe<real, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PipeSmem<real, N>::bytes);
+      const int pb = (int)PipeSmem<real, N>::bytes;
+      e = cudaFuncSetAttribute(k_pipe<real, N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pb);
       if (e != cudaSuccess) return (int)e;
-      e = cudaFuncSetAttribute(k_pipe<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PipeSmem<real, N>::bytes);
+      e = cudaFuncSetAttribute(k_pipe<real, N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pb);
+      if (e != cudaSuccess) return (int)e;
+      e = cudaFuncSetAttribute(k_pipe<real, N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pb);
+      if (e != cudaSuccess) return (int)e;
+      e = cudaFuncSetAttribute(k_pipe<real, N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pb);
       if (e != cudaSuccess) return (int)e;
     }
     if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled) {
@@ -113,12 +118,16 @@ template <typename real> struct Launch {
   static void pipe(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    launch_pdl(k_pipe<real, N, false>, a.nblk < g_sms ? a.nblk : g_sms, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    const int grid = a.nblk < g_sms ? a.nblk : g_sms;
+    if (a.sched_mode) launch_pdl(k_pipe<real, N, false, true>, grid, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    else launch_pdl(k_pipe<real, N, false, false>, grid, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void pipe2(const StepArgs& a, cudaStream_t s) {
     if (a.nblk <= 0) return;
     using C = PipeCfg<real, N>;
-    launch_pdl(k_pipe<real, N, true>, a.nblk < g_sms ? a.nblk : g_sms, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    const int grid = a.nblk < g_sms ? a.nblk : g_sms;
+    if (a.sched_mode) launch_pdl(k_pipe<real, N, true, true>, grid, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
+    else launch_pdl(k_pipe<real, N, true, false>, grid, C::G * C::NT * 32, PipeSmem<real, N>::bytes, s, a);
   }
   static void tc(const StepArgs& a, cudaStream_t s) {
     if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled) {

@@ -132,7 +132,7 @@ __device__ __forceinline__ void load_packed(const real* __restrict__ p, real (&o
 }
 
 
-template <typename real, int N, bool DUAL>
+template <typename real, int N, bool DUAL, bool TICKETS>
 __global__ void __launch_bounds__(PipeCfg<real, N>::G * PipeCfg<real, N>::NT * 32, 1)
 k_pipe(const __grid_constant__ StepArgs a) {
   using O = Order<N>;
@@ -201,33 +201,40 @@ k_pipe(const __grid_constant__ StepArgs a) {
   const real* myD = sD + (size_t)w * Np * RL;
   const real* myL = sL + (size_t)w * NF * LL;
 
-  // work distribution.  A group's j-th turn takes block base0 + j * stride while that is below `limit`, then blocks by
-  // ticket from a global counter (one atomic per block, taken three turns ahead).  sched_mode 0 (single-rate launches):
-  // fixed contiguous chunks per CTA, no tickets - the streams stay sequential and every block costs the same.
-  // sched_mode 1 (multi-rate launches): the first three turns interleaved over all groups, the rest by ticket - blocks
-  // differ in cost (levels, half-step traces) and sit sorted by level, so fixed chunks would load the SMs unevenly, and
-  // a launch of a few hundred blocks spreads over all SMs.  ring[j & 3] = block of the group's j-th turn, bend = none
+  // work distribution.  TICKETS = false (single-rate launches): fixed contiguous chunks per CTA, the groups of a CTA
+  // taking every G-th block of its chunk - the streams stay sequential and every block costs the same.  TICKETS = true
+  // (multi-rate launches): the first three turns of a group interleaved over all groups, then blocks by ticket from
+  // a global counter (one atomic per block, taken three turns ahead) - blocks differ in cost (levels, half-step
+  // traces) and sit sorted by level, so fixed chunks would load the SMs unevenly, and a launch of a few hundred blocks
+  // spreads over all SMs.  ring[j & 3] = block of the group's j-th turn (TICKETS only); bend = no block
   int* ring = reinterpret_cast<int*>(smem_raw + SM::ops_bytes + 96) + 4 * g;
   const int bend = a.blk0 + a.nblk, ngroups = (int)gridDim.x * G;
   const int lo = a.blk0 + (int)(((long long)a.nblk * blockIdx.x) / gridDim.x);
   const int hi = a.blk0 + (int)(((long long)a.nblk * (blockIdx.x + 1)) / gridDim.x);
-  const bool tickets = a.sched_mode != 0;
-  const int base0 = tickets ? a.blk0 + g * (int)gridDim.x + (int)blockIdx.x : lo + g;
-  const int stride = tickets ? ngroups : G;
+  const int base0 = a.blk0 + g * (int)gridDim.x + (int)blockIdx.x;
   const long long dyn0 = (long long)a.blk0 + 3LL * ngroups;
-  const int limit = tickets ? (dyn0 < bend ? (int)dyn0 : bend) : hi;
+  const int limit = dyn0 < bend ? (int)dyn0 : bend;
   unsigned* const ticket = a.sched + a.sched_sel;
   const real dir = (real)a.dir;
   const int n0 = w * TO;
 
-  auto item_block = [&](int i) { return ring[(i / NFLD) & 3]; };
+  const int nmine = (hi - lo - g + G - 1) / G;                    // fixed chunks: blocks of this group
+  const int nitems = nmine > 0 ? nmine * NFLD : 0;
+  auto item_block = [&](int i) {
+    if constexpr (TICKETS) return ring[(i / NFLD) & 3];
+    else return lo + g + (i / NFLD) * G;
+  };
+  auto has_item = [&](int i) {                                    // the group has an i-th item
+    if constexpr (TICKETS) return ring[(i / NFLD) & 3] < bend;
+    else return i < nitems;
+  };
   auto level_of = [&](int b) { int l = 0; while (b >= a.lv[l].blk_end) ++l; return l; };
   auto load_codes = [&](int i, int (&code)[FPW]) {
     const int b = item_block(i);
 #pragma unroll
     for (int k = 0; k < FPW; ++k) {
       const int f = w + k * NT;
-      code[k] = (f < 4 && b < bend) ? a.nbr[((size_t)b * 4 + f) * 32 + lane] : -1;
+      code[k] = (f < 4 && has_item(i)) ? a.nbr[((size_t)b * 4 + f) * 32 + lane] : -1;
     }
   };
   // everything item i needs, into stage s: bulk copies by one lane, trace records by their consumer lanes
@@ -316,11 +323,13 @@ k_pipe(const __grid_constant__ StepArgs a) {
   // on the stream and touches only what no launch writes (tables, neighbour codes); after it the previous launch's
   // results (q, right-hand sides, traces, ticket counter) are read
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (w == 0 && lane < 3) {                     // the first three turns
-    const int bs = base0 + lane * stride;
-    ring[lane] = bs < limit ? bs : bend;        // (with tickets the first three turns are always the fixed ones)
+  if constexpr (TICKETS) {
+    if (w == 0 && lane < 3) {                   // the first three turns
+      const int bs = base0 + lane * ngroups;
+      ring[lane] = bs < limit ? bs : bend;
+    }
+    group_sync<NT>(g);
   }
-  group_sync<NT>(g);
   load_codes(0, codeA);
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
@@ -330,16 +339,16 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
     for (int i2 = 0; i2 < Nfp; ++i2) fofs[k][i2] = (w + k * NT < 4 ? sF[(w + k * NT) * Nfp + i2] : 0) * 32 + lane;
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (blockIdx.x == 0 && tid == 0) a.sched[a.sched_sel ^ 1] = 0u;   // the next launch's counter (this launch's predecessor is done with it)
-  if (item_block(0) < bend) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
+  if (TICKETS && blockIdx.x == 0 && tid == 0) a.sched[a.sched_sel ^ 1] = 0u;   // the next launch's counter (this launch's predecessor is done with it)
+  if (has_item(0)) { issue_q(0, 0); issue_tr(0, codeA); issue_r(0); }
 
   unsigned tk = 0;
 #pragma unroll 1
-  for (int i = 0; item_block(i) < bend; ++i) {
+  for (int i = 0; has_item(i); ++i) {
     const int s = QS == 2 ? (i & 1) : 0, b = item_block(i), fi = i % NFLD, l = level_of(b);
-    const bool more = item_block(i + 1) < bend;                   // another item follows
+    const bool more = has_item(i + 1);                            // another item follows
     // ticket of the block three turns ahead: taken now, stored at the end of this block's last item
-    if (tickets && w == 0 && lane == 0 && fi == 0) tk = atomicAdd(ticket, 1u);
+    if (TICKETS && w == 0 && lane == 0 && fi == 0) tk = atomicAdd(ticket, 1u);
     const StepLevel& L = a.lv[l];
     real* Q = grp + (size_t)s * SM::stage_reals;                  // [4Np][32]
     const real* geo = Q + 4 * Np * 32 + lane;
@@ -764,9 +773,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
     }
 #pragma unroll
     for (int k = 0; k < FPW; ++k) { codeA[k] = codeB[k]; codeB[k] = codeC[k]; }
-    if (w == 0 && lane == 0 && fi == NFLD - 1) {                  // slot of the finished turn <- block three turns ahead
-      const long long bs = (long long)base0 + (long long)(i / NFLD + 3) * stride, nb = dyn0 + (long long)tk;
-      ring[(i / NFLD + 3) & 3] = tickets ? (nb < bend ? (int)nb : bend) : (bs < limit ? (int)bs : bend);
+    if (TICKETS && w == 0 && lane == 0 && fi == NFLD - 1) {       // slot of the finished turn <- block three turns ahead
+      const long long nb = dyn0 + (long long)tk;
+      ring[(i / NFLD + 3) & 3] = nb < bend ? (int)nb : bend;
     }
   }
   if constexpr (TMEM) {                         // every warp is done with its columns: release the tensor memory
