@@ -117,6 +117,16 @@ int dg_set_exterior(dg_ctx* ctx, const double* ext);
 int rtm_set_receiver_capacity(dg_ctx* ctx, int64_t max_receivers);   /* before rtm_history_bytes / rtm_bind_history */
 int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n);
 int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n);
+/* Boundary-trace spill to host memory for histories larger than HBM (the paper keeps the traces in host RAM / on disk,
+ * PAPER.md:399-407).  rtm_spill_bytes: host bytes of the whole trace history of shots of nsteps
+ * global steps.  rtm_set_trace_spill: `host` = caller-owned PINNED host memory of n bytes (borrowed until replaced or
+ * dg_destroy; NULL switches the spill off), `window` >= 2 = records of the coarsest level kept on the device (level l
+ * keeps window << l): the RTM region then holds that ring only, every captured record is copied to the host on a second
+ * stream behind the step that wrote it, and the backward phase fetches the records it replays window - 1 evaluations
+ * ahead.  Call before rtm_history_bytes / rtm_bind_history (it unbinds the RTM region).  Results are bit-identical to
+ * the in-HBM history. */
+int rtm_spill_bytes(dg_ctx* ctx, int nsteps, size_t* n);
+int rtm_set_trace_spill(dg_ctx* ctx, void* host, size_t n, int window);
 /* Forward phase: from rest at t = 0, source on, nsteps global steps; captures the boundary traces,
  * keeps q(t_f) on the device, records p(x_r, j dt_local), j = 0..nfine, into data_out[nr][nfine+1]
  * (host; may be NULL).  Synchronises. */

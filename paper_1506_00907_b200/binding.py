@@ -53,6 +53,8 @@ SIGNATURES = {
     "dg_step": (_i, [_vp, _i]),
     "dg_set_exterior": (_i, [_vp, _pd]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
+    "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
+    "rtm_set_trace_spill": (_i, [_vp, _vp, _sz, _i]),
     "rtm_history_bytes": (_i, [_vp, _i, _psz]),
     "rtm_bind_history": (_i, [_vp, _vp, _sz]),
     "rtm_forward_shot": (_i, [_vp, _i, _pd]),
@@ -197,6 +199,23 @@ class DG:
     # ---- RTM
     def rtm_set_receiver_capacity(self, max_receivers):
         self._ck(_lib.rtm_set_receiver_capacity(self._h, int(max_receivers)))
+
+    def rtm_spill_bytes(self, nsteps):
+        n = _sz()
+        self._ck(_lib.rtm_spill_bytes(self._h, int(nsteps), C.byref(n)))
+        return n.value
+
+    def rtm_set_trace_spill(self, host_ptr, nbytes, window):
+        self._ck(_lib.rtm_set_trace_spill(self._h, _vp(host_ptr), nbytes, int(window)))
+
+    def spill_traces_torch(self, nsteps, window):
+        """Pinned host tensor for the whole trace history; the RTM region bound afterwards keeps a ring of `window`."""
+        import torch
+        n = self.rtm_spill_bytes(nsteps)
+        self._spill = torch.empty(n + 64, dtype=torch.uint8, pin_memory=True)
+        base = (self._spill.data_ptr() + 15) & ~15
+        self.rtm_set_trace_spill(base, n, window)
+        return n
 
     def rtm_history_bytes(self, nsteps):
         n = _sz()

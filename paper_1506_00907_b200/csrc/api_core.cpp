@@ -272,6 +272,11 @@ void dg_destroy(dg_ctx* ctx) { delete ctx; }
 } // extern C
 dg_ctx::~dg_ctx() {
   for (dgrtm::ProfEvent& e : prof_ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  for (int l = 0; l < dgrtm::kMaxLevels; ++l) {
+    for (cudaEvent_t e : ev_step[l]) cudaEventDestroy(e);
+    for (cudaEvent_t e : ev_copy[l]) cudaEventDestroy(e);
+  }
+  if (copy_stream) cudaStreamDestroy(copy_stream);
 }
 extern "C" {
 

@@ -12,6 +12,43 @@ using namespace dgrtm;
 namespace {
 
 int64_t records_of_level(const dg_ctx* c, int l, int nsteps) { return ((int64_t)nsteps << l) + 1; }
+// records of level l the DEVICE holds: all of them, or a ring of spill_window << l when the history spills to the host
+int64_t device_records(const dg_ctx* c, int l, int nsteps) {
+  const int64_t all = records_of_level(c, l, nsteps);
+  return c->spill_window > 0 ? std::min<int64_t>(all, (int64_t)c->spill_window << l) : all;
+}
+size_t record_bytes(const dg_ctx* c, int l) { return c->model.stored[l].size() * (size_t)c->REC * c->rs; }
+size_t spill_host_bytes(const dg_ctx* c, int nsteps) {
+  size_t n = 0;
+  for (int l = 0; l < c->model.nlevels; ++l) n += ((size_t)records_of_level(c, l, nsteps) * record_bytes(c, l) + 255) / 256 * 256;
+  return n;
+}
+void spill_release(dg_ctx* c) {
+  for (int l = 0; l < kMaxLevels; ++l) {
+    for (cudaEvent_t e : c->ev_step[l]) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_copy[l]) cudaEventDestroy(e);
+    c->ev_step[l].clear(); c->ev_copy[l].clear(); c->slot_rec[l].clear();
+  }
+}
+// ring bookkeeping of a bound history: which record every slot holds, one event pair per slot
+void spill_setup(dg_ctx* c, int nsteps) {
+  spill_release(c);
+  if (c->spill_window <= 0) return;
+  if (!c->copy_stream) cuda_check(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate (trace spill)");
+  size_t off = 0;
+  for (int l = 0; l < c->model.nlevels; ++l) {
+    c->hrec[l] = c->spill_host + off;
+    off += ((size_t)records_of_level(c, l, nsteps) * record_bytes(c, l) + 255) / 256 * 256;
+    const int64_t W = device_records(c, l, nsteps);
+    c->slot_rec[l].assign((size_t)W, -1);
+    c->ev_step[l].resize((size_t)W); c->ev_copy[l].resize((size_t)W);
+    for (int64_t x = 0; x < W; ++x) {
+      cuda_check(cudaEventCreateWithFlags(&c->ev_step[l][x], cudaEventDisableTiming), "cudaEventCreate");
+      cuda_check(cudaEventCreateWithFlags(&c->ev_copy[l][x], cudaEventDisableTiming), "cudaEventCreate");
+      cudaEventRecord(c->ev_copy[l][x], c->copy_stream);      // "no transfer pending"
+    }
+  }
+}
 
 void group_receivers(dg_ctx* c) {
   const Model& md = c->model;
@@ -38,7 +75,7 @@ void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
   const size_t rs = c->rs;
   const int Np = c->Np;
   for (int l = 0; l < md.nlevels; ++l)
-    c->rec[l] = cv.take((size_t)records_of_level(c, l, nsteps) * md.stored[l].size() * c->REC * rs);
+    c->rec[l] = cv.take((size_t)device_records(c, l, nsteps) * md.stored[l].size() * c->REC * rs);
   const size_t nr = (size_t)std::max<int64_t>(1, std::max(c->nr, c->nr_reserve));   // receiver capacity
   c->d_data = cv.take(nr * ((size_t)nsteps * c->nlocal + 1) * rs);
   c->d_rcv_slot = (int*)cv.take(nr * 4);
@@ -108,6 +145,53 @@ void copy_data(dg_ctx* c, double* host, const double* host_in, int64_t ncol) {
 }  // namespace
 
 namespace dgrtm {
+char* record_ptr(dg_ctx* c, int l, int64_t j) {
+  const int64_t slot = c->spill_window > 0 ? j % (int64_t)c->slot_rec[l].size() : j;
+  return c->rec[l] + (size_t)slot * record_bytes(c, l);
+}
+// forward: the slot of record j may be overwritten once its previous occupant has reached the host
+void spill_before_capture(dg_ctx* c, int l, int64_t j) {
+  if (c->spill_window <= 0) return;
+  const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size());
+  cuda_check(cudaStreamWaitEvent(c->stream, c->ev_copy[l][slot], 0), "cudaStreamWaitEvent");
+  c->slot_rec[l][slot] = j;
+}
+// forward: record j is complete when the launch that captured it is: send it to the host behind the compute stream
+void spill_after_capture(dg_ctx* c, int l, int64_t j) {
+  if (c->spill_window <= 0) return;
+  const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size()), nb = record_bytes(c, l);
+  cuda_check(cudaEventRecord(c->ev_step[l][slot], c->stream), "cudaEventRecord");
+  cuda_check(cudaStreamWaitEvent(c->copy_stream, c->ev_step[l][slot], 0), "cudaStreamWaitEvent");
+  cuda_check(cudaMemcpyAsync(c->hrec[l] + (size_t)j * nb, c->rec[l] + slot * nb, nb, cudaMemcpyDeviceToHost, c->copy_stream), "trace record D2H");
+  cuda_check(cudaEventRecord(c->ev_copy[l][slot], c->copy_stream), "cudaEventRecord");
+}
+namespace {
+// make record j of level l resident in its ring slot (no-op if it is there or on its way); the bound stream does not wait
+void spill_fetch(dg_ctx* c, int l, int64_t j) {
+  const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size()), nb = record_bytes(c, l);
+  if (c->slot_rec[l][slot] == j) return;
+  cuda_check(cudaStreamWaitEvent(c->copy_stream, c->ev_step[l][slot], 0), "cudaStreamWaitEvent");   // its last reader is done
+  cuda_check(cudaMemcpyAsync(c->rec[l] + slot * nb, c->hrec[l] + (size_t)j * nb, nb, cudaMemcpyHostToDevice, c->copy_stream), "trace record H2D");
+  cuda_check(cudaEventRecord(c->ev_copy[l][slot], c->copy_stream), "cudaEventRecord");
+  c->slot_rec[l][slot] = j;
+}
+}  // namespace
+// backward: record j must be in its slot before the launch that replays it
+void spill_before_replay(dg_ctx* c, int l, int64_t j) {
+  if (c->spill_window <= 0) return;
+  spill_fetch(c, l, j);
+  const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size());
+  cuda_check(cudaStreamWaitEvent(c->stream, c->ev_copy[l][slot], 0), "cudaStreamWaitEvent");
+}
+// backward: the launch that replayed record j is queued; its slot's next occupant, and the records the coming launches
+// need, are fetched behind it (the ring keeps W - 1 records ahead of the replay)
+void spill_after_replay(dg_ctx* c, int l, int64_t j) {
+  if (c->spill_window <= 0) return;
+  const int64_t W = (int64_t)c->slot_rec[l].size();
+  const size_t slot = (size_t)(j % W);
+  cuda_check(cudaEventRecord(c->ev_step[l][slot], c->stream), "cudaEventRecord");
+  for (int64_t k = 1; k < W; ++k) { if (j - k < 0) break; spill_fetch(c, l, j - k); }
+}
 void upload_receiver_tables(dg_ctx* ctx) {
   group_receivers(ctx);
   const int64_t nr = ctx->nr;
@@ -151,6 +235,26 @@ int rtm_image_device(dg_ctx* ctx, void** dptr, size_t* nbytes) {
   DG_CATCH(ctx)
 }
 
+int rtm_spill_bytes(dg_ctx* ctx, int nsteps, size_t* n) {
+  DG_TRY(ctx)
+  if (!n) throw ApiError(DG_ERR_ARG, "n is NULL");
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  if (nsteps < 1) throw ApiError(DG_ERR_ARG, "nsteps must be >= 1");
+  *n = spill_host_bytes(ctx, nsteps);
+  DG_CATCH(ctx)
+}
+
+int rtm_set_trace_spill(dg_ctx* ctx, void* host, size_t n, int window) {
+  DG_TRY(ctx)
+  if (host && window < 2) throw ApiError(DG_ERR_ARG, "window must be >= 2 records");
+  if (host && ((uintptr_t)host & 15) != 0) throw ApiError(DG_ERR_ARG, "host buffer must be 16-byte aligned");
+  if (ctx->bound) sync_stream(ctx);
+  if (ctx->copy_stream) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
+  ctx->spill_host = (char*)host; ctx->spill_bytes = host ? n : 0; ctx->spill_window = host ? window : 0;
+  ctx->hist_bound = false;                     // the record layout of the RTM region changed: bind it again
+  DG_CATCH(ctx)
+}
+
 int rtm_history_bytes(dg_ctx* ctx, int nsteps, size_t* n) {
   DG_TRY(ctx)
   if (!n) throw ApiError(DG_ERR_ARG, "n is NULL");
@@ -175,7 +279,10 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
     HistPtrs keep;
     keep.save(ctx);
     int lo = 0, hi = 1;
-    auto fits = [&](int s) { Carver cnt; carve_history(ctx, cnt, s); return cnt.used <= n; };
+    auto fits = [&](int s) {
+      Carver cnt; carve_history(ctx, cnt, s);
+      return cnt.used <= n && (ctx->spill_window <= 0 || spill_host_bytes(ctx, s) <= ctx->spill_bytes);
+    };
     if (fits(1)) {
       lo = 1;
       while (hi < (1 << 28) && fits(hi * 2)) hi *= 2;
@@ -190,6 +297,7 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
   Carver cv;
   cv.base = ctx->hs;
   carve_history(ctx, cv, nsteps);
+  spill_setup(ctx, nsteps);
   ctx->nr_cap = std::max(ctx->nr, ctx->nr_reserve);
   upload_receiver_tables(ctx);
   ctx->hist_bound = true;
@@ -218,6 +326,7 @@ int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out) {
   ctx->data_valid = ctx->nr > 0;
   if (data_out) copy_data(ctx, data_out, nullptr, (int64_t)nsteps * ctx->nlocal + 1);
   sync_stream(ctx);
+  if (ctx->spill_window > 0) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
   DG_CATCH(ctx)
 }
 
@@ -296,7 +405,14 @@ int rtm_get_traces(dg_ctx* ctx, int level, int64_t record, double* buf) {
   if (record < 0 || record >= records_of_level(ctx, level, ctx->hist_nsteps)) throw ApiError(DG_ERR_ARG, "record out of range");
   const size_t nf = ctx->model.stored[level].size(), Nfp = ctx->Nfp;
   std::vector<double> tmp(nf * 2 * Nfp);
-  download_real(ctx, tmp.data(), ctx->rec[level] + (size_t)record * nf * ctx->REC * ctx->rs, tmp.size());
+  if (ctx->spill_window > 0) {                 // the host copy is the history
+    sync_stream(ctx);
+    cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
+    const char* src = ctx->hrec[level] + (size_t)record * nf * ctx->REC * ctx->rs;
+    for (size_t i = 0; i < tmp.size(); ++i) tmp[i] = ctx->precision == 64 ? ((const double*)src)[i] : (double)((const float*)src)[i];
+  } else {
+    download_real(ctx, tmp.data(), ctx->rec[level] + (size_t)record * nf * ctx->REC * ctx->rs, tmp.size());
+  }
   // device record: [face][p | n.v][Nfp]  ->  buf[face][Nfp][2]
   for (size_t x = 0; x < nf; ++x)
     for (size_t i = 0; i < Nfp; ++i) {

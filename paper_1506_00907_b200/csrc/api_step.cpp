@@ -51,9 +51,6 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   for (int l = 0; l < L; ++l) stride[l] = 1 << (L - 1 - l);
   const int src_level = c->has_src ? md.level[c->src_k] : -1;
   const int64_t nsamp = (int64_t)c->hist_nsteps * nloc + 1;
-  auto record_ptr = [&](int l, int64_t j) -> char* {
-    return c->rec[l] + (size_t)j * md.stored[l].size() * c->REC * c->rs;
-  };
   // p(x_r) at fine time m BEFORE the launch of fine step m: a level at its step start holds q(t); a level
   // in mid-step already holds q at the END of its step: p(t) = q_end - dt_l sum_s (a_s - I_s(theta)) r_s
   // with the interpolant (22) (reading Q13)
@@ -131,8 +128,10 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       for (int s = 0; s < 3; ++s) { S.c[s] = dts * co.a[s]; S.d[s] = dts * (co.b[s] - co.a[s]); S.abar[s] = co.abar[s]; }
       for (int s = 0; s < 9; ++s) S.C[s] = co.C[s];
       const bool stored = !md.stored[l].empty();
-      S.capture = (o.capture && stored) ? record_ptr(l, jabs / stride[l]) : nullptr;
-      S.replay = (o.replay && stored) ? record_ptr(l, jabs / stride[l]) : nullptr;
+      S.capture = (o.capture && stored) ? record_ptr(c, l, jabs / stride[l]) : nullptr;
+      S.replay = (o.replay && stored) ? record_ptr(c, l, jabs / stride[l]) : nullptr;
+      if (S.capture) spill_before_capture(c, l, jabs / stride[l]);
+      if (S.replay) spill_before_replay(c, l, jabs / stride[l]);
       const int64_t jlast = jabs + dir * (stride[l] - 1);   // start of the fine step on which this update lands
       S.image_on = o.image && std::min(jlast, jlast + dir) >= o.image_min_fine;
     }
@@ -145,8 +144,11 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, pipe ? c->kt->pipe2(a, c->stream) : c->kt->step2(a, c->stream));
       else DG_LAUNCH(c, KC_STEP, tc ? c->kt->tc(a, c->stream) : (pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream)));
     }
-    for (int l = lmin; l < L; ++l)
+    for (int l = lmin; l < L; ++l) {
+      if (a.lv[l].capture) spill_after_capture(c, l, jabs / stride[l]);
+      if (a.lv[l].replay) spill_after_replay(c, l, jabs / stride[l]);
       for (int fi = 0; fi < o.nfields; ++fi) o.fields[fi]->par[l] ^= 1;
+    }
   }
   const int64_t jend = o.first_fine + dir * nfine;
   if (o.capture) {
@@ -155,8 +157,10 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       CaptureArgs ca;
       std::memset(&ca, 0, sizeof(ca));
       ca.q = o.fields[0]->q; ca.geo = c->geo; ca.faces = c->d_stored[l]; ca.nfaces = (int)md.stored[l].size();
-      ca.record = record_ptr(l, jend / stride[l]); ca.ops = c->ops;
+      ca.record = record_ptr(c, l, jend / stride[l]); ca.ops = c->ops;
+      spill_before_capture(c, l, jend / stride[l]);
       DG_LAUNCH(c, KC_CAPTURE, c->kt->capture(ca, c->stream));
+      spill_after_capture(c, l, jend / stride[l]);
     }
   }
   if (o.record && c->nr > 0) sample_receivers(0, jend);

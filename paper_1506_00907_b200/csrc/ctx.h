@@ -157,6 +157,16 @@ struct dg_ctx {
   char* qfinal = nullptr;
   bool have_final = false, have_backward = false;
   int final_nsteps = 0;
+  // ---- boundary-trace spill to host memory (off by default): the device
+  // keeps a ring of spill_window << level records per level, the whole history lives in caller-owned pinned host memory
+  char* spill_host = nullptr;
+  size_t spill_bytes = 0;
+  int spill_window = 0;                     // records of the coarsest level on the device; 0 = no spill
+  char* hrec[dgrtm::kMaxLevels];            // per level: the host copy [nrec][nfaces][2][Nfp]
+  cudaStream_t copy_stream = nullptr;
+  std::vector<int64_t> slot_rec[dgrtm::kMaxLevels];   // record held (or being loaded) by every ring slot, -1 = none
+  std::vector<cudaEvent_t> ev_step[dgrtm::kMaxLevels];   // bound stream: the launch that wrote / read the slot
+  std::vector<cudaEvent_t> ev_copy[dgrtm::kMaxLevels];   // copy stream: the slot's last transfer
 
   int64_t launches = 0;
   // per-kernel timing (dg_set_profiling): one CUDA event pair per launch on the bound stream
@@ -186,6 +196,13 @@ void normalize_traces(dg_ctx* c, Field& F);
 void upload_point_source(dg_ctx* c);        // per-slot point-term index of the forward field // current traces of every level -> qfb[0] (= qf)
 void clear_field(dg_ctx* c, Field& F);
 void upload_receiver_tables(dg_ctx* c);     // receiver rows / weights / groups -> the bound RTM region
+// trace records: device address of record j of level l (a ring slot when the history spills to the host), and the
+// stream choreography around the launch that captures (forward) or replays (backward) it
+char* record_ptr(dg_ctx* c, int l, int64_t j);
+void spill_before_capture(dg_ctx* c, int l, int64_t j);
+void spill_after_capture(dg_ctx* c, int l, int64_t j);
+void spill_before_replay(dg_ctx* c, int l, int64_t j);
+void spill_after_replay(dg_ctx* c, int l, int64_t j);
 void restart_history(dg_ctx* c);            // after dg_set_integrator / dg_set_dt
 
 struct RunOpts {

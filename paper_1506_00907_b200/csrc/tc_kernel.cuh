@@ -25,6 +25,9 @@ template <int N> struct TcCfg { static constexpr bool enabled = false; static co
 #define DG_TC3_G 3
 #endif
 template <> struct TcCfg<3> { static constexpr bool enabled = true; static constexpr int G = DG_TC3_G; };
+#ifdef DG_TC4
+template <> struct TcCfg<4> { static constexpr bool enabled = true; static constexpr int G = 1; };
+#endif
 
 template <int N> struct TcSmem {
   using O = Order<N>;
