@@ -475,7 +475,7 @@ def measured_alu_peaks(device, peak_hbm):
             "fused_step_bound_by_order": binds}
 
 
-def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps):
+def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps, traffic_table=None):
     """One full RTM shot of config 4 through the C ABI (host data buffers): forward with trace capture
     and receiver recording, backward with trace replay, receiver injection and fused imaging."""
     from workloads import make_config
@@ -504,7 +504,8 @@ def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps):
         if n:
             nbytes = float(nb) * fields * g.K * algorithmic_scalars(name, g.Np, g.Nfp) * rs
             ker[name] = {"launches": n, "avg_us": round(ms * 1e3 / n, 2), "achieved_gbs": round(nbytes / ms * 1e-6, 1),
-                         "frac": round(nbytes / ms * 1e-6 / peak, 4)}
+                         "frac": round(nbytes / ms * 1e-6 / peak, 4),
+                         "traffic": traffic_of(traffic_table or {}, "cfg4_rtm", cfg["N"], cfg["precision"], name) if hexes is None else None}
     out = {"workload": "cfg4_rtm", "K": int(g.K), "N": cfg["N"], "dtype": "f%d" % cfg["precision"], "nsteps": nsteps,
            "receivers": int(g.nr), "forward_s": t1 - t0, "backward_s": t2 - t1, "image_read_s": t3 - t2,
            "shot_s": t3 - t0, "forward_dof_updates_per_s": dof * nsteps / (t1 - t0),
@@ -691,7 +692,7 @@ def run_ours(args):
         line["unfused_kernels"] = extra_unfused_kernels(torch, device, peak, None if big else (8, 8, 4), traffic_table)
         line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8))
         line["rtm_shot"] = extra_rtm_shot(torch, device, peak, peak_src, None if big else (8, 8, 4),
-                                          None if big else 20)
+                                          None if big else 20, traffic_table)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:

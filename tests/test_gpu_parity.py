@@ -457,11 +457,13 @@ def test_full_size_rtm_two_steps():
         g.close()
 
 
-def test_tensor_core_variant_is_close_but_opt_in(monkeypatch):
-    """The tcgen05 / tensor-memory variant of the step kernel (DGRTM_KERNEL=tc, fp32 N = 3, 3xTF32 split) is NOT the
-    default: it does not hold the 1e-5 fp32 tolerance over a 1000-step run (1.4e-5 measured on config 2) and is not
-    faster.  It must still be a correct implementation of the same step to TF32x3 accuracy."""
-    cfg = make_config("cfg2_two_layer", hexes=(6, 5, 4), nsteps=200)
+@pytest.mark.parametrize("N", [3, 4])
+def test_tensor_core_variant_is_close_but_opt_in(N, monkeypatch):
+    """The tcgen05 / tensor-memory variant of the step kernel (DGRTM_KERNEL=tc, fp32, N = 3 and 4, 3xTF32 split) is NOT
+    the default: it does not hold the 1e-5 fp32 tolerance over a 1000-step run (1.4e-5 measured on config 2) and is not
+    faster (N = 4: one group per SM, the split A operand fills the tensor memory).  It must still be a
+    correct implementation of the same step to TF32x3 accuracy."""
+    cfg = make_config("cfg2_two_layer", hexes=(6, 5, 4), N=N, nsteps=200)
     cfg["source"] = dict(cfg["source"], f0=40.0, tp=0.005)
     o = make_oracle(cfg)
     monkeypatch.setenv("DGRTM_KERNEL", "tc")
