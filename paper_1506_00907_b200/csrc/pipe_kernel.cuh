@@ -82,7 +82,7 @@ template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; sta
 #define DG_D3_G 3
 #endif
 #ifndef DG_D3_TP
-#define DG_D3_TP 1
+#define DG_D3_TP 2
 #endif
 #ifndef DG_D3_OFF
 template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0, F2 = 0, TP = DG_D3_TP; };
@@ -174,7 +174,9 @@ k_pipe(const __grid_constant__ StepArgs a) {
   constexpr int PCOLS = PCOLS_NEED <= 32 ? 32 : (PCOLS_NEED <= 64 ? 64 : (PCOLS_NEED <= 128 ? 128 : (PCOLS_NEED <= 256 ? 256 : 512)));
   static_assert(PCOLS_NEED <= 512, "tensor memory has 512 columns");
   constexpr bool TMEM = PARK || IPARK;
-  constexpr int PCN = (TO + 3) / 4;                               // nodes per chunk: one chunk per face of the lift loop
+  // two register buffers alternating (five chunks, two faces of latency each) or one (four chunks, one face each)
+  constexpr bool PARK2 = PARK && Cfg::TP == 2 && !DUAL;
+  constexpr int PCN = PARK2 ? (TO + 4) / 5 : (TO + 3) / 4;        // nodes per chunk
   unsigned* tmem_slot = reinterpret_cast<unsigned*>(bars + 3 * G + 1);
 
   {  // operator tables + Fmask + permutation table: one blob, laid out on the host exactly as here
@@ -546,12 +548,15 @@ k_pipe(const __grid_constant__ StepArgs a) {
       }
     }
     group_sync<NT>(g);                          // every warp has read Q: the update may overwrite its tile's nodes
-    // ---- surface (Alg. 3, second half); with PARK, chunk f of the older right-hand sides (h1, h2 of PCN of this
-    // warp's nodes, 4 fields) is in flight from L2 during the lift of face f and parked in tensor memory after it
+    // ---- surface (Alg. 3, second half).  With PARK the older right-hand sides (h1, h2 of this warp's nodes, 4 fields)
+    // come from L2 in chunks of PCN nodes and are parked in tensor memory.  One buffer (TP = 1): chunk f is in flight
+    // during the lift of face f.  Two alternating buffers (TP = 2, fp64 N = 3 where one face is shorter than the L2 round
+    // trip): chunk 0 is requested before the loop into A, chunk f + 1 at the start of face f (into B for even f, A for
+    // odd f), and a buffer is parked just before it is reused or after the loop - two faces to land
     const real* h1g = static_cast<const real*>(L.r1[fi]) + base + (size_t)n0 * 32;
     const real* h2g = static_cast<const real*>(L.r2[fi]) + base + (size_t)n0 * 32;
-    real hc[PARK ? PCN : 1][8];
-    auto load_chunk = [&](int c) {
+    real hA[PARK ? PCN : 1][8], hB[PARK2 ? PCN : 1][8];
+    auto load_chunk = [&](int c, real (&hc)[PARK ? PCN : 1][8]) {
 #pragma unroll
       for (int j = 0; j < PCN; ++j) {
         const int nn = c * PCN + j;
@@ -564,7 +569,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
         }
       }
     };
-    auto park_chunk = [&](int c) {
+    auto park_chunk = [&](int c, const real (&hc)[PARK ? PCN : 1][8]) {   // (hB has this extent only with PARK2, its only user)
 #pragma unroll
       for (int j = 0; j < PCN; ++j) {
         const int nn = c * PCN + j;
@@ -575,9 +580,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
         }
       }
     };
-    if constexpr (PARK) load_chunk(0);
-#pragma unroll 1
-    for (int f = 0; f < 4; ++f) {
+    auto lift_face = [&](int f) {
       real av[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) av[nn] = 0;
@@ -604,10 +607,32 @@ k_pipe(const __grid_constant__ StepArgs a) {
       const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { rx[nn] -= nx * av[nn]; ry[nn] -= ny * av[nn]; rz[nn] -= nz * av[nn]; }
-      if constexpr (PARK) {
-        park_chunk(f);
-        if (f + 1 < 4) load_chunk(f + 1);
+    };
+    if constexpr (PARK && !PARK2) {               // one buffer: chunk f in flight during the lift of face f
+      load_chunk(0, hA);
+#pragma unroll 1
+      for (int f = 0; f < 4; ++f) {
+        lift_face(f);
+        park_chunk(f, hA);
+        if (f + 1 < 4) load_chunk(f + 1, hA);
       }
+    } else if constexpr (PARK2) {
+      load_chunk(0, hA);
+#pragma unroll 1
+      for (int fp = 0; fp < 2; ++fp) {
+        const int f = 2 * fp;
+        if (fp > 0) park_chunk(f - 1, hB);        // chunk f - 1, requested at the start of face f - 2
+        load_chunk(f + 1, hB);
+        lift_face(f);
+        park_chunk(f, hA);                        // chunk f, requested at the start of face f - 1 (chunk 0: before the loop)
+        load_chunk(f + 2, hA);
+        lift_face(f + 1);
+      }
+      park_chunk(3, hB);
+      park_chunk(4, hA);
+    } else {
+#pragma unroll 1
+      for (int f = 0; f < 4; ++f) lift_face(f);
     }
     if constexpr (PARK) tmem_wait_st();
 
