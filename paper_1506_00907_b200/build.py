@@ -52,7 +52,6 @@ def build(force=False, orders=(1, 2, 3, 4, 5, 6), verbose=False):
         objs.append(obj)
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
             jobs.append([NVCC, "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xptxas", "-v", "-DDG_ORDER=%d" % n,
-                         *os.environ.get("DG_NVCC_FLAGS", "").split(),     # tuning sweeps (-DDG_F3_TO=.. etc.)
                          "-Xcompiler", "-fPIC", "-c", src, "-o", obj])
     for name in CUDA_SOURCES:          # order-independent device code
         src = os.path.join(CSRC, name)

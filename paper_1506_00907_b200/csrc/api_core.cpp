@@ -188,6 +188,26 @@ void fields_from_device(dg_ctx* c, double* q, const char* dq) {
   else unpack_fields(c, q, reinterpret_cast<const float*>(tmp.data()));
 }
 
+// user order I[K][Np] <- device [block][Np][32], one threaded pass from the device precision
+void image_from_device(dg_ctx* c, double* I, const char* dimg) {
+  const int Np = c->Np;
+  std::vector<char> tmp((size_t)c->model.nblocks * Np * 32 * c->rs);
+  cuda_check(cudaMemcpyAsync(tmp.data(), dimg, tmp.size(), cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
+  sync_stream(c);
+  const bool f64 = c->precision == 64;
+  const char* base = tmp.data();
+  parallel_slots(c->model.nslots, [&](int64_t s0, int64_t s1) {
+    for (int64_t s = s0; s < s1; ++s) {
+      const int64_t k = c->model.elem_of[s];
+      if (k < 0) continue;
+      const size_t o = (size_t)(s >> 5) * Np * 32 + (size_t)(s & 31);
+      double* out = I + (size_t)k * Np;
+      if (f64) { const double* in = reinterpret_cast<const double*>(base) + o; for (int n = 0; n < Np; ++n) out[n] = in[(size_t)n * 32]; }
+      else { const float* in = reinterpret_cast<const float*>(base) + o; for (int n = 0; n < Np; ++n) out[n] = (double)in[(size_t)n * 32]; }
+    }
+  });
+}
+
 void clear_field(dg_ctx* c, Field& F) {
   cuda_check(cudaMemsetAsync(F.q, 0, field_bytes(c), c->stream), "memset q");
   for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(F.hist[s], 0, field_bytes(c), c->stream), "memset hist");

@@ -370,14 +370,7 @@ int rtm_image_read(dg_ctx* ctx, double* I_out) {
   DG_TRY(ctx)
   require_history(ctx);
   if (!I_out) throw ApiError(DG_ERR_ARG, "I_out is NULL");
-  const int Np = ctx->Np;
-  std::vector<double> tmp((size_t)ctx->model.nblocks * Np * 32);
-  download_real(ctx, tmp.data(), ctx->image, tmp.size());
-  for (int64_t s = 0; s < ctx->model.nslots; ++s) {
-    const int64_t k = ctx->model.elem_of[s];
-    if (k < 0) continue;
-    for (int n = 0; n < Np; ++n) I_out[(size_t)k * Np + n] = tmp[(((size_t)(s >> 5)) * Np + n) * 32 + (s & 31)];
-  }
+  image_from_device(ctx, I_out, ctx->image);
   DG_CATCH(ctx)
 }
 

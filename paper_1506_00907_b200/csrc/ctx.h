@@ -191,6 +191,7 @@ void sync_stream(dg_ctx* c);
 // user order q[K][4][Np]  <->  device [block][4Np][32]
 void fields_to_device(dg_ctx* c, char* dq, const double* q);
 void fields_from_device(dg_ctx* c, double* q, const char* dq);
+void image_from_device(dg_ctx* c, double* I, const char* dimg);   // user order I[K][Np] <- device [block][Np][32]
 void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
 void normalize_traces(dg_ctx* c, Field& F);
 void upload_point_source(dg_ctx* c);        // per-slot point-term index of the forward field // current traces of every level -> qfb[0] (= qf)

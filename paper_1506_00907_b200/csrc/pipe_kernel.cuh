@@ -14,79 +14,22 @@
 
 namespace dgrtm {
 
-// TO outputs per warp, NT warps per block, G groups per CTA, QS = stages of the q ring (2: fetched one item
-// ahead; 1: fetched at the start of the item from L2, where a prefetch issued one item ahead has put it)
-// RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: read from global in the
-// update phase after an L2 prefetch (saves 8Np rows of shared memory per group: more groups per SM)
+// Tiling and staging of one (precision, order); the values are the winners of the sweeps in profiles/r1b, r2_experiments:
+//   TO outputs per warp, NT warps per block, G groups per CTA;
+//   QS = stages of the q ring (2: fetched one item ahead; 1: requested during the previous item's trace write-out, from
+//        L2, where a prefetch issued one item ahead has put it);
+//   RS = 1: the two older right-hand sides go through shared memory (bulk copy); 0: no room for them there;
+//   TP (with RS = 0): they are loaded from L2 in chunks during the lift loop and PARKED in tensor memory (tcgen05.st; lane =
+//        element, columns = values), from where the update reads them back (tcgen05.ld) - shared memory and the register
+//        file are full, the 256 KB of tensor memory are idle.  1: one chunk buffer, 2: two alternating (one-field kernel);
+//   UG = 1: velocities -> U.G once per block, in place in shared memory; 0: every warp forms U.G on the fly (9 more FMAs
+//        per input node and warp, two shared-memory passes and one barrier fewer);
+//   F2 = 1: the volume contraction uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the FMA instructions for twice the
+//        accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 857 -> 911 us).
 template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0, TP = 0; };
-// F2 = 1: the volume contraction of the one-field fp32 kernel uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the
-// FMA instructions for twice the accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 977 -> 1020 us)
-// TP = 1 (with RS = 0): the two older right-hand sides of the warp's own output nodes are loaded from L2 in chunks
-// during the lift loop and PARKED in tensor memory (tcgen05.st; lane = element, columns = values), from where the update
-// reads them back (tcgen05.ld): shared memory and the register file are full, the 256 KB of tensor memory are idle
-// UG = 1: velocities -> U.G once per block, in place in shared memory; 0: every warp forms U.G on the fly
-// (9 more FMAs per input node and warp, two shared-memory passes and one barrier fewer)
-#ifndef DG_PIPE_FFMA2
-#define DG_PIPE_FFMA2 1
-#endif
-#ifndef DG_PIPE_FFMA2_DUAL
-#define DG_PIPE_FFMA2_DUAL 1
-#endif
-#ifndef DG_P3_TO
-#define DG_P3_TO 5
-#endif
-#ifndef DG_P3_NT
-#define DG_P3_NT 4
-#endif
-#ifndef DG_P3_G
-#define DG_P3_G 3
-#endif
-#ifndef DG_P3_RS
-#define DG_P3_RS 1
-#endif
-#ifndef DG_P3_QS
-#define DG_P3_QS 2
-#endif
-#ifndef DG_P3_UG
-#define DG_P3_UG 0
-#endif
-template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_P3_TO, NT = DG_P3_NT, G = DG_P3_G, QS = DG_P3_QS, RS = DG_P3_RS, UG = DG_P3_UG, F2 = DG_PIPE_FFMA2, TP = 0; };
-#ifndef DG_P4_TO
-#define DG_P4_TO 9
-#endif
-#ifndef DG_P4_NT
-#define DG_P4_NT 4
-#endif
-#ifndef DG_P4_G
-#define DG_P4_G 3
-#endif
-#ifndef DG_P4_RS
-#define DG_P4_RS 0
-#endif
-#ifndef DG_P4_UG
-#define DG_P4_UG 0
-#endif
-#ifndef DG_P4_TP
-#define DG_P4_TP 1
-#endif
-#ifndef DG_P4_F2
-#define DG_P4_F2 0
-#endif
-#ifndef DG_P4_QS
-#define DG_P4_QS 1
-#endif
-template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = DG_P4_TO, NT = DG_P4_NT, G = DG_P4_G, QS = DG_P4_QS, RS = DG_P4_RS, UG = DG_P4_UG, F2 = DG_P4_F2, TP = DG_P4_TP; };
-#ifndef DG_D3_TO
-#define DG_D3_TO 5
-#define DG_D3_NT 4
-#define DG_D3_G 3
-#endif
-#ifndef DG_D3_TP
-#define DG_D3_TP 2
-#endif
-#ifndef DG_D3_OFF
-template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = DG_D3_TO, NT = DG_D3_NT, G = DG_D3_G, QS = 1, RS = 0, UG = 0, F2 = 0, TP = DG_D3_TP; };
-#endif
+template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 2, RS = 1, UG = 0, F2 = 1, TP = 0; };
+template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = 9, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
+template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
 
 template <typename real, int N> struct PipeSmem {
   using O = Order<N>;
@@ -476,7 +419,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
 
     // ---- volume (eqs (13)-(14), Alg. 2)
     real rp[TO], rx[TO], ry[TO], rz[TO];
-    if constexpr (sizeof(real) == 4 && Cfg::F2 && (!DUAL || DG_PIPE_FFMA2_DUAL)) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
+    if constexpr (sizeof(real) == 4 && Cfg::F2) {  // packed fp32x2 FMAs (sm_100): one instruction per pair of row entries
                                                  // (the two-field kernel is register-bound and keeps scalar FMAs)
       float2 aG2[RL / 2], aD2[RL / 2];
 #pragma unroll
@@ -517,10 +460,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
       real aD[TO], aR[TO], aS[TO], aT[TO];
 #pragma unroll
       for (int nn = 0; nn < TO; ++nn) { aD[nn] = 0; aR[nn] = 0; aS[nn] = 0; aT[nn] = 0; }
-#ifndef DG_PIPE_UNROLL_M
-#define DG_PIPE_UNROLL_M 5
-#endif
-      constexpr int UM = DG_PIPE_UNROLL_M;
+      constexpr int UM = 5;
 #pragma unroll UM
       for (int m = 0; m < Np; ++m) {
         const real p = Q[m * 32 + lane];

@@ -21,33 +21,20 @@
 
 namespace dgrtm {
 
-#ifndef DG_STEP_PARK
-#define DG_STEP_PARK 1
-#endif
 template <typename real, int N> struct StepCfg;
 //                                            TO = outputs per warp, NT = warps per block, G = groups per CTA,
 //                                            PK = older right-hand sides parked in tensor memory (N = 5 fp32: the
 //                                            96-register budget of its 21 warps has no room for the chunk in flight)
 template <> struct StepCfg<float, 1> { static constexpr int TO = 4, NT = 1, G = 16, PK = 1; };
 template <> struct StepCfg<float, 2> { static constexpr int TO = 12, NT = 1, G = 12, PK = 1; };
-#ifndef DG_F3_TO
-#define DG_F3_TO 10
-#define DG_F3_NT 2
-#define DG_F3_G 10
-#endif
-template <> struct StepCfg<float, 3> { static constexpr int TO = DG_F3_TO, NT = DG_F3_NT, G = DG_F3_G, PK = 1; };
+template <> struct StepCfg<float, 3> { static constexpr int TO = 10, NT = 2, G = 10, PK = 1; };
 template <> struct StepCfg<float, 4> { static constexpr int TO = 12, NT = 3, G = 5, PK = 1; };
 template <> struct StepCfg<float, 5> { static constexpr int TO = 8, NT = 7, G = 3, PK = 0; };
 template <> struct StepCfg<float, 6> { static constexpr int TO = 12, NT = 7, G = 2, PK = 1; };
 template <> struct StepCfg<double, 1> { static constexpr int TO = 4, NT = 1, G = 12, PK = 1; };
 template <> struct StepCfg<double, 2> { static constexpr int TO = 10, NT = 1, G = 8, PK = 1; };
 template <> struct StepCfg<double, 3> { static constexpr int TO = 10, NT = 2, G = 5, PK = 1; };
-#ifndef DG_S4D_TO
-#define DG_S4D_TO 6
-#define DG_S4D_NT 6
-#define DG_S4D_G 2
-#endif
-template <> struct StepCfg<double, 4> { static constexpr int TO = DG_S4D_TO, NT = DG_S4D_NT, G = DG_S4D_G, PK = 1; };
+template <> struct StepCfg<double, 4> { static constexpr int TO = 6, NT = 6, G = 2, PK = 1; };
 template <> struct StepCfg<double, 5> { static constexpr int TO = 8, NT = 7, G = 1, PK = 1; };
 template <> struct StepCfg<double, 6> { static constexpr int TO = 12, NT = 7, G = 1, PK = 1; };
 
@@ -251,7 +238,7 @@ k_step(const __grid_constant__ StepArgs a) {
   // the two older right-hand sides of the warp's own output nodes are loaded from L2 in chunks during the lift loop
   // and PARKED in tensor memory (lane = element, columns = values; idle otherwise), where the update finds them
   // without a global-load latency: per warp 8 TO reals, warps of one lane quarter side by side
-  constexpr bool PARK = DG_STEP_PARK != 0 && Cfg::PK;
+  constexpr bool PARK = Cfg::PK != 0;
   constexpr int PW = Words8<real>::NW;                            // 32-bit columns per node
   constexpr int PCOLS_NEED = (G * NT + 3) / 4 * TO * PW;
   constexpr int PCOLS = PCOLS_NEED <= 32 ? 32 : (PCOLS_NEED <= 64 ? 64 : (PCOLS_NEED <= 128 ? 128 : (PCOLS_NEED <= 256 ? 256 : 512)));

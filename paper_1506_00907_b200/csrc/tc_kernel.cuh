@@ -21,10 +21,7 @@
 namespace dgrtm {
 
 template <int N> struct TcCfg { static constexpr bool enabled = false; static constexpr int G = 1; };
-#ifndef DG_TC3_G
-#define DG_TC3_G 3
-#endif
-template <> struct TcCfg<3> { static constexpr bool enabled = true; static constexpr int G = DG_TC3_G; };
+template <> struct TcCfg<3> { static constexpr bool enabled = true; static constexpr int G = 3; };
 // N = 4: the 3xTF32 split of A needs 2 x 112 + 48 = 272 of the 512 tensor-memory columns per group: one group per SM
 // (N >= 5 does not fit at all: 2 x 184 + 64 columns at N = 5 leave no second group, N = 6 needs 608)
 template <> struct TcCfg<4> { static constexpr bool enabled = true; static constexpr int G = 1; };
