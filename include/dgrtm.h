@@ -110,6 +110,29 @@ int dg_step(dg_ctx* ctx, int nsteps);
  * right-hand side until replaced.  Entries of faces of another type are ignored. */
 int dg_set_exterior(dg_ctx* ctx, const double* ext);
 
+/* ---- domain decomposition, single-rate -----------------------
+ * A sub-domain is an ordinary ctx over its part of the mesh whose cut faces are DG_BC_PRESCRIBED faces.  Their exterior
+ * state is the neighbouring sub-domain's exposed trace at the coinciding node, fetched on the DEVICE by dg_halo_pull
+ * straight from the neighbour's trace buffer (its own ctx on this GPU, or a peer pointer over NVLink): no host staging.
+ * dg_set_exterior_impedance: Zext[nbnd] = rho c of the element behind each boundary face (<= 0: none; NULL: clear), so
+ *   that a halo face gets the same single-valued impedance (Z- + Z+) / 2 as the interior face it replaces (reading Q4);
+ *   call before dg_workspace_bytes / dg_bind_workspace (it unbinds).
+ * dg_get_slots: slot_of[K], the position of every element in the level-sorted device order (a trace record of face f
+ *   of element k is record slot_of[k] * 4 + f of the trace buffer: p[Nfp] then n.v[Nfp], own face-node order on
+ *   boundary faces).
+ * dg_get_trace_device: device pointer / size of the buffer that holds the exposed traces at the current time (it
+ *   alternates between two buffers from step to step: query it before every dg_halo_pull).
+ * dg_set_halo: halo set `set` (0..7, one per neighbouring sub-domain, filled in ascending order) of nh faces:
+ *   bnd_index[nh] (boundary-face-list index here), src_record[nh] (record in that neighbour's buffer), src_pos[nh][Nfp]
+ *   (position in that record of the node coinciding with my face node i).  After bind.
+ * dg_halo_pull: enqueue the fetch of one set on this ctx's stream (the caller orders it after the neighbour's last step).
+ * A time step of the decomposed problem = every sub-domain pulls, then every sub-domain takes dg_step(1). */
+int dg_set_exterior_impedance(dg_ctx* ctx, const double* Zext);
+int dg_get_slots(dg_ctx* ctx, int64_t* slot_of);
+int dg_get_trace_device(dg_ctx* ctx, void** dptr, size_t* nbytes);
+int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, const int64_t* src_record, const int32_t* src_pos);
+int dg_halo_pull(dg_ctx* ctx, int set, const void* src_trace_device);
+
 /* ---- RTM (Fig. 1) ---------------------------------------------------
  * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side
  * evaluation time of its owner plus the final time (layout reading Q12) - it stays in
@@ -194,7 +217,7 @@ int dg_get_launch_count(const dg_ctx* ctx, int64_t* n);
  * a CUDA event pair on the bound stream (adds ~2 us per launch; off by default).  dg_get_kernel_times
  * synchronises, sums the elapsed milliseconds and the launch counts per kernel class since the last
  * call into ms[DG_KC_COUNT], count[DG_KC_COUNT] and forgets the events. */
-enum { DG_KC_RHS = 0, DG_KC_UPDATE, DG_KC_HALF, DG_KC_IMAGE_UPDATE, DG_KC_SOURCE, DG_KC_RECORD,
+enum { DG_KC_RHS = 0, DG_KC_UPDATE, DG_KC_HALO, DG_KC_IMAGE_UPDATE, DG_KC_SOURCE, DG_KC_RECORD,
        DG_KC_INJECT, DG_KC_CAPTURE, DG_KC_RK, DG_KC_STEP, DG_KC_STEP_IMAGE, DG_KC_COUNT };
 int dg_set_profiling(dg_ctx* ctx, int on);
 int dg_get_kernel_times(dg_ctx* ctx, double* ms, int64_t* count);

@@ -26,7 +26,7 @@ DG_WAVELET_RICKER = 0
 DG_IMAGING_CLASSICAL, DG_IMAGING_CHARACTERISTIC = 0, 1
 DG_IMAGING_CLASSICAL_TRAPEZOID, DG_IMAGING_CHARACTERISTIC_TRAPEZOID = 2, 3
 DG_RHS_VOLUME, DG_RHS_SURFACE, DG_RHS_TOTAL = 0, 1, 2
-KERNEL_CLASSES = ("rhs", "update", "unused", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
+KERNEL_CLASSES = ("rhs", "update", "halo", "image_update", "source", "record", "inject", "capture", "rk", "step", "step_image")
 
 _vp, _i, _i64, _d, _sz = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_size_t
 _pd = C.POINTER(C.c_double)
@@ -52,6 +52,11 @@ SIGNATURES = {
     "dg_set_state": (_i, [_vp, _pd, _d]),
     "dg_step": (_i, [_vp, _i]),
     "dg_set_exterior": (_i, [_vp, _pd]),
+    "dg_set_exterior_impedance": (_i, [_vp, _pd]),
+    "dg_get_slots": (_i, [_vp, _pi64]),
+    "dg_get_trace_device": (_i, [_vp, C.POINTER(_vp), C.POINTER(_sz)]),
+    "dg_set_halo": (_i, [_vp, _i, _i64, _pi32, _pi64, _pi32]),
+    "dg_halo_pull": (_i, [_vp, _i, _vp]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
     "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
     "rtm_set_trace_spill": (_i, [_vp, _vp, _sz, _i]),
@@ -195,6 +200,33 @@ class DG:
         ext = _f64(ext)
         assert ext.shape == (self.nbnd, self.Nfp, 2)
         self._ck(_lib.dg_set_exterior(self._h, _ptr(ext, _pd)))
+
+    # ---- domain decomposition (halo faces)
+    def dg_set_exterior_impedance(self, Zext):
+        Zext = None if Zext is None else _f64(Zext)
+        assert Zext is None or Zext.shape == (self.nbnd,)
+        self._ck(_lib.dg_set_exterior_impedance(self._h, _ptr(Zext, _pd)))
+
+    def dg_get_slots(self):
+        s = np.empty(self.K, dtype=np.int64)
+        self._ck(_lib.dg_get_slots(self._h, _ptr(s, _pi64)))
+        return s
+
+    def dg_get_trace_device(self):
+        p, n = _vp(), _sz()
+        self._ck(_lib.dg_get_trace_device(self._h, C.byref(p), C.byref(n)))
+        return p.value, n.value
+
+    def dg_set_halo(self, halo_set, bnd_index, src_record, src_pos):
+        bnd_index = np.ascontiguousarray(bnd_index, dtype=np.int32)
+        src_record = np.ascontiguousarray(src_record, dtype=np.int64)
+        src_pos = np.ascontiguousarray(src_pos, dtype=np.int32)
+        assert src_record.shape == bnd_index.shape and src_pos.shape == (bnd_index.size, self.Nfp)
+        self._ck(_lib.dg_set_halo(self._h, int(halo_set), int(bnd_index.size), _ptr(bnd_index, _pi32), _ptr(src_record, _pi64),
+                                  _ptr(src_pos, _pi32)))
+
+    def dg_halo_pull(self, halo_set, src_trace_device):
+        self._ck(_lib.dg_halo_pull(self._h, int(halo_set), _vp(src_trace_device)))
 
     # ---- RTM
     def rtm_set_receiver_capacity(self, max_receivers):

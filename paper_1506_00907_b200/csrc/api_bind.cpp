@@ -137,6 +137,10 @@ void upload_tables(dg_ctx* c) {
       g[(GEO_FACE + 5 * f + 3) * 32] = m.gsur[4 * k + f];
       // single-valued face impedance (reading Q4)
       g[(GEO_FACE + 5 * f + 4) * 32] = k2 >= 0 ? 0.5 * (Z + md.rho[k2] * md.c[k2]) : Z;
+      if (k2 < 0 && !c->bnd_Zext.empty()) {        // halo face: the neighbouring sub-domain's impedance (dg_set_exterior_impedance)
+        const double Ze = c->bnd_Zext[m.bnd_index[4 * k + f]];
+        if (Ze > 0) g[(GEO_FACE + 5 * f + 4) * 32] = 0.5 * (Z + Ze);
+      }
       int32_t code;
       if (k2 >= 0) {
         code = (int32_t)(md.slot_of[k2] * 4 + m.EToF[4 * k + f]);
@@ -196,7 +200,7 @@ int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream) {
   cuda_check(cudaMemsetAsync(ctx->ws, 0, need, ctx->stream), "cudaMemsetAsync workspace");
   upload_tables(ctx);
   ctx->F.reset_history();
-  ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false;
+  ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false; for (int x = 0; x < 9; ++x) ctx->halo_off[x] = 0;
   ctx->have_final = false; ctx->have_backward = false;
   sync_stream(ctx);
   DG_CATCH(ctx)
@@ -212,6 +216,89 @@ int dg_set_state(dg_ctx* ctx, const double* q, double t0) {
   refresh_traces(ctx, ctx->F);
   ctx->t0 = t0; ctx->fine = 0;
   sync_stream(ctx);
+  DG_CATCH(ctx)
+}
+
+// ---- domain decomposition: halo faces -----------------------------
+int dg_set_exterior_impedance(dg_ctx* ctx, const double* Zext) {
+  DG_TRY(ctx)
+  const size_t nb = ctx->mesh.bnd_k.size();
+  if (Zext) ctx->bnd_Zext.assign(Zext, Zext + nb); else ctx->bnd_Zext.clear();
+  ctx->bound = false; ctx->hist_bound = false;   // the face impedances live in the bound factors: bind again
+  DG_CATCH(ctx)
+}
+
+int dg_get_slots(dg_ctx* ctx, int64_t* slot_of) {
+  DG_TRY(ctx)
+  if (!slot_of) throw ApiError(DG_ERR_ARG, "slot_of is NULL");
+  if (!ctx->has_model) throw ApiError(DG_ERR_STATE, "dg_set_model first");
+  for (int64_t k = 0; k < ctx->mesh.K; ++k) slot_of[k] = ctx->model.slot_of[k];
+  DG_CATCH(ctx)
+}
+
+int dg_get_trace_device(dg_ctx* ctx, void** dptr, size_t* nbytes) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!dptr || !nbytes) throw ApiError(DG_ERR_ARG, "dptr / nbytes is NULL");
+  if (ctx->model.nlevels != 1) throw ApiError(DG_ERR_UNSUPPORTED, "the halo exchange is single-rate");
+  *dptr = ctx->F.qfb[ctx->F.par[0]];
+  *nbytes = trace_bytes(ctx);
+  DG_CATCH(ctx)
+}
+
+int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, const int64_t* src_record, const int32_t* src_pos) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  const int64_t nb = (int64_t)ctx->mesh.bnd_k.size();
+  const int Nfp = ctx->Nfp;
+  if (set < 0 || set > 7) throw ApiError(DG_ERR_ARG, "halo set must be in 0..7");
+  const int64_t h0 = ctx->halo_off[set];          // sets are filled in ascending order: set s starts where s - 1 ended
+  if (nh < 0 || h0 + nh > nb) throw ApiError(DG_ERR_ARG, "more halo faces than boundary faces");
+  if (nh && (!bnd_index || !src_record || !src_pos)) throw ApiError(DG_ERR_ARG, "NULL table");
+  if (ctx->model.nlevels != 1) throw ApiError(DG_ERR_UNSUPPORTED, "the halo exchange is single-rate");
+  for (int64_t h = 0; h < nh; ++h) {
+    const int32_t bi = bnd_index[h];
+    if (bi < 0 || bi >= nb) throw ApiError(DG_ERR_ARG, "boundary-face index out of range");
+    if (ctx->mesh.bc[4 * (size_t)ctx->mesh.bnd_k[bi] + ctx->mesh.bnd_f[bi]] != DG_BC_PRESCRIBED)
+      throw ApiError(DG_ERR_ARG, "halo faces must be DG_BC_PRESCRIBED faces");
+    if (src_record[h] < 0) throw ApiError(DG_ERR_ARG, "negative source record");
+    for (int i = 0; i < Nfp; ++i)
+      if (src_pos[h * Nfp + i] < 0 || src_pos[h * Nfp + i] >= Nfp) throw ApiError(DG_ERR_ARG, "source node position out of range");
+  }
+  // carved region: [bnd int32 nb | pad to 8 | rec int64 nb | pos int32 nb*Nfp], the sets one after the other
+  char* base = ctx->d_halo;
+  const size_t off_rec = ((size_t)nb * 4 + 7) / 8 * 8, off_pos = off_rec + (size_t)nb * 8;
+  if (nh) {
+    upload_raw(ctx, base + (size_t)h0 * 4, bnd_index, (size_t)nh * 4);
+    upload_raw(ctx, base + off_rec + (size_t)h0 * 8, src_record, (size_t)nh * 8);
+    upload_raw(ctx, base + off_pos + (size_t)h0 * Nfp * 4, src_pos, (size_t)nh * Nfp * 4);
+  }
+  if (!ctx->has_ext) {   // prescribed faces that are no halo faces keep a zero exterior until dg_set_exterior
+    cuda_check(cudaMemsetAsync(ctx->ext, 0, std::max<size_t>(1, (size_t)nb) * Nfp * 2 * ctx->rs, ctx->stream), "memset ext");
+    ctx->has_ext = true;
+  }
+  for (int x = set + 1; x < 9; ++x) ctx->halo_off[x] = h0 + nh;
+  DG_CATCH(ctx)
+}
+
+int dg_halo_pull(dg_ctx* ctx, int set, const void* src_trace_device) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (set < 0 || set > 7) throw ApiError(DG_ERR_ARG, "halo set must be in 0..7");
+  if (!src_trace_device) throw ApiError(DG_ERR_ARG, "source trace buffer is NULL");
+  const int64_t h0 = ctx->halo_off[set], nh = ctx->halo_off[set + 1] - h0;
+  if (nh > 0) {
+    const size_t nb = ctx->mesh.bnd_k.size();
+    const size_t off_rec = (nb * 4 + 7) / 8 * 8, off_pos = off_rec + nb * 8;
+    HaloArgs a;
+    a.src_qf = src_trace_device; a.ext = ctx->ext;
+    a.bnd = reinterpret_cast<const int*>(ctx->d_halo) + h0;
+    a.rec = reinterpret_cast<const long long*>(ctx->d_halo + off_rec) + h0;
+    a.pos = reinterpret_cast<const int*>(ctx->d_halo + off_pos) + (size_t)h0 * ctx->Nfp;
+    a.nh = (int)nh;
+    DG_LAUNCH(ctx, KC_HALO, ctx->kt->halo(a, ctx->stream));
+    check_launches(ctx);
+  }
   DG_CATCH(ctx)
 }
 

@@ -427,6 +427,7 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
   c->scratch = cv.take(field_bytes(c));
   c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);
   c->d_src_w = cv.take((size_t)Np * rs);
+  c->d_halo = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * (size_t)(4 + 8 + 4 * Nfp) + 64);   // halo tables (dg_set_halo)
   for (int l = 0; l < md.nlevels; ++l) {
     c->d_stored[l] = (int*)cv.take(std::max<size_t>(1, md.stored[l].size()) * 4);
   }
@@ -452,13 +453,13 @@ int dg_workspace_bytes(dg_ctx* ctx, size_t* n) {
   {
     // the carve writes pointers into the ctx: save and restore them so a bound ctx is not disturbed
     OpsDev ops = ctx->ops; char* geo = ctx->geo; int* nbr = ctx->nbr; int* wperm = ctx->wperm; Field F = ctx->F;
-    char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w;
+    char* scratch = ctx->scratch; char* ext = ctx->ext; char* sw = ctx->d_src_w; char* dh = ctx->d_halo;
     char* dp = ctx->d_D3P; char* lp = ctx->d_LTP; char* dq = ctx->d_D3Q; char* lq = ctx->d_LTQ; unsigned char* bf = ctx->d_blkflag; int* ps = ctx->d_pt_src;
     int* ds[kMaxLevels];
     for (int l = 0; l < kMaxLevels; ++l) ds[l] = ctx->d_stored[l];
     carve_workspace(ctx, count);
     ctx->ops = ops; ctx->geo = geo; ctx->nbr = nbr; ctx->wperm = wperm; ctx->F = F;
-    ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw;
+    ctx->scratch = scratch; ctx->ext = ext; ctx->d_src_w = sw; ctx->d_halo = dh;
     ctx->d_D3P = dp; ctx->d_LTP = lp; ctx->d_D3Q = dq; ctx->d_LTQ = lq; ctx->d_blkflag = bf; ctx->d_pt_src = ps;
     for (int l = 0; l < kMaxLevels; ++l) ctx->d_stored[l] = ds[l];
   }

@@ -18,7 +18,7 @@ namespace dgrtm {
 constexpr int kMaxLevels = 8;
 
 // kernel classes of the launch counter / per-kernel timing (dg_get_kernel_times)
-enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALF, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_STEP, KC_STEP_IMAGE, KC_COUNT };
+enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALO, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_STEP, KC_STEP_IMAGE, KC_COUNT };
 struct ProfEvent { cudaEvent_t a, b; int cls; };
 
 struct ApiError : std::runtime_error {
@@ -132,6 +132,10 @@ struct dg_ctx {
   unsigned char* d_blkflag = nullptr;       // per block: bit 0 = some element has a finer face neighbour; then the ticket counters
   int sched_sel = 0;                        // ticket counter the next pipelined launch uses (the kernel zeroes the other one)
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
+  // ---- halo faces of a domain decomposition (dg_set_halo): tables [bnd | rec | pos] in one carved region
+  char* d_halo = nullptr;
+  int64_t halo_off[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // faces of halo set s (one set per neighbouring sub-domain): [halo_off[s], halo_off[s+1])
+  std::vector<double> bnd_Zext;             // exterior impedance per boundary face (> 0: Z_f = (Z- + Zext) / 2), dg_set_exterior_impedance
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
   int64_t fine = 0;                         // time = t0 + fine * dt_local

@@ -422,6 +422,23 @@ __global__ void k_capture(CaptureArgs a) {
   rec[Nfp + i] = gf[0] * q[o + (size_t)Np * 32] + gf[32] * q[o + (size_t)2 * Np * 32] + gf[64] * q[o + (size_t)3 * Np * 32];
 }
 
+// halo exchange of a domain decomposition ("transfer the traces of fields situated at the interface
+// between two sub-domains"): the cut faces are prescribed-exterior faces here; their exterior state (p+, n-.v+) is the
+// neighbouring sub-domain's exposed trace at the coinciding node, with n-.v+ = -(n+.v+) (reading Q6b).  src_qf may be
+// a peer pointer: the loads then cross NVLink, nothing is staged on the host
+template <typename real, int N>
+__global__ void k_halo(HaloArgs a) {
+  constexpr int Nfp = Order<N>::Nfp, REC = Order<N>::REC;
+  const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tid >= (long)a.nh * Nfp) return;
+  const int h = (int)(tid / Nfp), i = (int)(tid - (long)h * Nfp);
+  const real* r = static_cast<const real*>(a.src_qf) + (size_t)a.rec[h] * REC;
+  const int j = a.pos[tid];
+  real* e = static_cast<real*>(a.ext) + ((size_t)a.bnd[h] * Nfp + i) * 2;
+  e[0] = r[j];
+  e[1] = -r[Nfp + j];
+}
+
 // -------------------------------------------------------------------------------------------------
 // point terms (eq (15))
 template <typename real, int N>

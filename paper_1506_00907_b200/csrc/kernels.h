@@ -92,6 +92,15 @@ struct CaptureArgs {       // own traces of a list of (slot*4+f) faces -> record
   const void* q; const void* geo; const int* faces; int nfaces; void* record; OpsDev ops;
 };
 
+struct HaloArgs {          // exterior states of halo faces <- exposed traces of the neighbouring sub-domain
+  const void* src_qf;        // the neighbour's trace buffer [slot][4][2][Nfp] (a peer pointer over NVLink, or local)
+  void* ext;                 // this sub-domain's prescribed-exterior array [nbnd][Nfp][2]
+  const int* bnd;            // [nh] boundary-face-list index of the halo face here
+  const long long* rec;      // [nh] record (slot * 4 + f) of the same face in the neighbour's buffer
+  const int* pos;            // [nh][Nfp] position in that record of the node that coincides with my face node i
+  int nh;
+};
+
 // ---- fused step kernel (step_kernel.cuh) ---------------------------------------------------------
 // One launch advances every level that sits at the start of the fine step.  Per level (contiguous block
 // range): where its right-hand sides rotate, where its traces are read / written, its AB weights.
@@ -146,6 +155,7 @@ struct KernelTable {
   void (*record)(const PointArgs&, cudaStream_t);
   void (*inject)(const PointArgs&, cudaStream_t);
   void (*capture)(const CaptureArgs&, cudaStream_t);
+  void (*halo)(const HaloArgs&, cudaStream_t);
   void (*step)(const StepArgs&, cudaStream_t);        // one wavefield
   void (*step2)(const StepArgs&, cudaStream_t);       // two wavefields + imaging
   int step_npad;                                       // padded output count of the step kernel's tables

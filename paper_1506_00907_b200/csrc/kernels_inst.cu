@@ -145,6 +145,11 @@ template <typename real> struct Launch {
     const long n = (long)a.ng * Order<N>::Np;
     k_inject<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
   }
+  static void halo(const HaloArgs& a, cudaStream_t s) {
+    if (a.nh <= 0) return;
+    const long n = (long)a.nh * Order<N>::Nfp;
+    k_halo<real, N><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(a);
+  }
   static void capture(const CaptureArgs& a, cudaStream_t s) {
     if (a.nfaces <= 0) return;
     const long n = (long)a.nfaces * Order<N>::Nfp;
@@ -162,7 +167,7 @@ template <typename real> KernelTable make_table(int precision) {
   t.rhs = Launch<real>::rhs; t.update = Launch<real>::update; t.rk = Launch<real>::rk;
   t.image_update = Launch<real>::image_update;
   t.source = Launch<real>::source; t.record = Launch<real>::record; t.inject = Launch<real>::inject;
-  t.capture = Launch<real>::capture; t.init = Launch<real>::init; t.take_error = Launch<real>::take_error;
+  t.capture = Launch<real>::capture; t.halo = Launch<real>::halo; t.init = Launch<real>::init; t.take_error = Launch<real>::take_error;
   t.pipe = nullptr; t.pipe2 = nullptr; t.pipe_TO = t.pipe_NT = t.pipe_RL = t.pipe_LL = 0; t.pipe_blob_bytes = 0;
   t.tc = nullptr; t.tc_K1 = t.tc_K2 = t.tc_NN = 0; t.tc_blob_bytes = 0;
   if constexpr (sizeof(real) == 4 && TcCfg<N>::enabled && TcSmem<N>::fits) {

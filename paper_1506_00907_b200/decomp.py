@@ -1,0 +1,150 @@
+"""Domain decomposition of the single-rate scheme over several sub-domains:
+set-up only - partition, local meshes, halo tables.  Every step of the path still runs in the library's kernels: a
+sub-domain is an ordinary `DG` context whose cut faces are prescribed-exterior faces, and their exterior states are
+fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_halo) before every step.
+
+    part = partition_elements(EToV, VX, nparts, weights)         # weighted recursive coordinate bisection
+    dd = Decomposition(N, precision, EToV, VX, rho, c, part)     # one DG context per part, halo tables
+    dd.bind_torch("cuda:0"); dd.dg_set_source(...); dd.dg_step(n); q = dd.dg_get_fields()
+
+The paper partitions with METIS, cell weights 2^(l-1) and keeps the finest cells off the cuts
+(PAPER.md:387); METIS is not in this container: `partition_elements` is a weighted coordinate bisection that takes the same
+weights.  Here all sub-domains live in one process (on one GPU their launches are ordered by the shared stream); with one
+process per GPU the source pointer of `dg_halo_pull` is a peer mapping of the neighbour's trace buffer and the loads
+cross NVLink - that launch mode needs more than the one GPU this pool grants and is not exercised.
+"""
+import numpy as np
+
+from .binding import DG
+
+BC_PRESCRIBED = 4
+
+
+def partition_elements(EToV, VX, nparts, weights=None):
+    """Part id per element by recursive coordinate bisection of the element centroids along the longest axis, each cut
+    balancing the summed weights (weight = local steps per global step of the cell)."""
+    K = EToV.shape[0]
+    cen = VX[EToV].mean(axis=1)
+    w = np.ones(K) if weights is None else np.asarray(weights, dtype=np.float64)
+    part = np.zeros(K, dtype=np.int32)
+
+    def split(idx, p0, n):
+        if n == 1:
+            part[idx] = p0
+            return
+        ext = cen[idx].max(axis=0) - cen[idx].min(axis=0)
+        order = idx[np.argsort(cen[idx, int(np.argmax(ext))], kind="stable")]
+        nl = n // 2
+        cw = np.cumsum(w[order])
+        cut = int(np.searchsorted(cw, cw[-1] * nl / n)) + 1
+        cut = min(max(cut, 1), len(order) - 1)
+        split(order[:cut], p0, nl)
+        split(order[cut:], p0 + nl, n - nl)
+
+    split(np.arange(K), 0, int(nparts))
+    return part
+
+
+class Decomposition:
+    """The sub-domains of one mesh as DG contexts with their halo tables.  Global arrays in, global arrays out."""
+
+    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15):
+        EToV = np.ascontiguousarray(EToV, dtype=np.int32)
+        self.K, self.part = EToV.shape[0], np.asarray(part, dtype=np.int32)
+        self.nparts = int(self.part.max()) + 1
+        assert self.nparts <= 9, "a sub-domain has at most 8 halo sets"
+        # global connectivity and the global stable step from a host-only context of the whole mesh
+        g = DG(N, precision, EToV, VX, face_bc=face_bc, default_bc=default_bc)
+        g.dg_set_model(rho, c, 1, cfl)
+        EToE, EToF, mapP = g.dg_get_connectivity()
+        self.dt = g.dg_get_dt()[0]
+        self.Np, self.Nfp = g.Np, g.Nfp
+        g.close()
+        self.elems = [np.nonzero(self.part == p)[0] for p in range(self.nparts)]
+        local = np.full(self.K, -1, dtype=np.int64)
+        for e in self.elems:
+            local[e] = np.arange(e.size)
+        self.local = local
+        self.sub, self._halo = [], []
+        Z = np.asarray(rho, dtype=np.float64) * np.asarray(c, dtype=np.float64)
+        for p, e in enumerate(self.elems):
+            verts, inv = np.unique(EToV[e], return_inverse=True)
+            etov = inv.reshape(-1, 4).astype(np.int32)
+            nb = EToE[e]                                              # [Kp][4] global neighbour or -1
+            cut = (nb >= 0) & (self.part[np.maximum(nb, 0)] != p)
+            fbc = np.full((e.size, 4), default_bc, dtype=np.int8) if face_bc is None else np.array(face_bc[e], dtype=np.int8)
+            fbc[cut] = BC_PRESCRIBED
+            s = DG(N, precision, etov, VX[verts], face_bc=fbc, default_bc=default_bc)
+            s.dg_set_model(np.asarray(rho)[e], np.asarray(c)[e], 1, cfl)
+            bk, bf, bc = s.dg_get_boundary_faces()
+            k2 = nb[bk, bf]                                           # global neighbour behind every boundary face
+            halo = (k2 >= 0) & (bc == BC_PRESCRIBED)
+            s.dg_set_exterior_impedance(np.where(halo, Z[np.maximum(k2, 0)], 0.0))
+            self.sub.append(s)
+            self._halo.append((bk, bf, k2, halo))
+        self._tables(EToF, mapP)
+        self._bound = False
+
+    def _tables(self, EToF, mapP):
+        slots = [s.dg_get_slots() for s in self.sub]
+        self.sets = []                                               # per sub-domain: list of (neighbour part, tables)
+        for p, s in enumerate(self.sub):
+            bk, bf, k2, halo = self._halo[p]
+            ge = self.elems[p][bk]                                    # global element of every boundary face
+            sets = []
+            for q in range(self.nparts):
+                sel = np.nonzero(halo & (self.part[np.maximum(k2, 0)] == q))[0]
+                if q == p or sel.size == 0:
+                    continue
+                f2 = EToF[ge[sel], bf[sel]]
+                rec = slots[q][self.local[k2[sel]]] * 4 + f2
+                pos = mapP[ge[sel], bf[sel]]                          # [nh][Nfp]: neighbour's face node at my node i
+                sets.append((q, sel.astype(np.int32), rec.astype(np.int64), pos.astype(np.int32)))
+            assert len(sets) <= 8
+            self.sets.append(sets)
+
+    # ---- memory, set-up
+    def bind_torch(self, device="cuda:0"):
+        for p, s in enumerate(self.sub):
+            s.bind_torch(device)
+            s.dg_set_dt(self.dt)                                      # the global stable step, not the sub-domain's own
+            for i, (q, bnd, rec, pos) in enumerate(self.sets[p]):
+                s.dg_set_halo(i, bnd, rec, pos)
+        self._bound = True
+
+    def dg_set_source(self, x0, f0, tp, amp=1.0):
+        """The point source goes to the sub-domain that contains it (lowest part id on a tie)."""
+        for s in self.sub:
+            try:
+                s.dg_set_source(x0, f0, tp, amp)
+                return
+            except Exception:
+                continue
+        raise ValueError("source outside the mesh")
+
+    def dg_set_state(self, q, t0=0.0):
+        for p, s in enumerate(self.sub):
+            s.dg_set_state(q[self.elems[p]], t0)
+
+    def dg_get_fields(self):
+        q = np.empty((self.K, 4, self.Np))
+        for p, s in enumerate(self.sub):
+            q[self.elems[p]] = s.dg_get_fields()
+        return q
+
+    # ---- the step: every sub-domain pulls its halo, then every sub-domain advances
+    def dg_step(self, nsteps):
+        for _ in range(int(nsteps)):
+            src = [s.dg_get_trace_device()[0] for s in self.sub]
+            for p, s in enumerate(self.sub):
+                for i, (q, _, _, _) in enumerate(self.sets[p]):
+                    s.dg_halo_pull(i, src[q])
+            for s in self.sub:
+                s.dg_step(1)
+
+    def launch_count(self):
+        return sum(s.dg_get_launch_count() for s in self.sub)
+
+    def close(self):
+        for s in self.sub:
+            s.close()
