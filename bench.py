@@ -516,6 +516,38 @@ def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps, traffic_table=N
     return out
 
 
+def extra_decomposition(torch, device, hexes, T=200):
+    """Config 2 cut into 2 and 4 sub-domains that step in lock-step on this one GPU (decomp.py: halo fetch by k_halo from
+    the neighbour's trace buffer, then one step per sub-domain): what the decomposition itself costs - smaller launches
+    and the halo kernels - before any NVLink is involved (one GPU in this pool)."""
+    from workloads import make_config
+    from paper_1506_00907_b200.decomp import Decomposition, partition_elements
+    cfg = make_config("cfg2_two_layer", hexes=hexes)
+    out = []
+    for nparts in (1, 2, 4):
+        part = partition_elements(cfg["EToV"], cfg["VX"], nparts)
+        dd = Decomposition(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
+                           default_bc=cfg["default_bc"], cfl=cfg["cfl"])
+        dd.bind_torch(device)
+        s = cfg["source"]
+        dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+        dd.dg_step(20)
+        torch.cuda.synchronize(device)
+        n0 = dd.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        dd.dg_step(T)
+        e1.record()
+        torch.cuda.synchronize(device)
+        us = e0.elapsed_time(e1) * 1e3 / T
+        halo = sum(sum(len(t[1]) for t in sets) for sets in dd.sets)
+        out.append({"sub_domains": nparts, "elements": [int(len(e)) for e in dd.elems], "halo_faces": int(halo),
+                    "us_per_time_step": round(us, 2), "launches_per_time_step": (dd.launch_count() - n0) / T,
+                    "value": 4 * dd.K * dd.Np / (us * 1e-6), "unit": UNIT})
+        dd.close()
+    return out
+
+
 def survey_shots(nshots, lengths, hexes, receivers):
     """Seeded shot list of a survey over one mesh ("29 gathers"): sources along a line at the top, each
     with its own receiver set (a shifted sub-grid, so the counts differ between gathers)."""
@@ -691,6 +723,7 @@ def run_ours(args):
                                                {} if big else {"cfg4_rtm": (8, 8, 4), "cfg3_lts": (8, 8, 8)}, traffic_table)
         line["unfused_kernels"] = extra_unfused_kernels(torch, device, peak, None if big else (8, 8, 4), traffic_table)
         line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8))
+        line["decomposition_one_gpu"] = extra_decomposition(torch, device, None if big else (8, 8, 4), 200 if big else 10)
         line["rtm_shot"] = extra_rtm_shot(torch, device, peak, peak_src, None if big else (8, 8, 4),
                                           None if big else 20, traffic_table)
     if rank == 0:
