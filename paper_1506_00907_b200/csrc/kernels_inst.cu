@@ -67,7 +67,7 @@ template <typename real> struct Launch {
     e = cudaFuncSetAttribute(k_step<real, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)StepSmem<real, N, true>::bytes);
     if (e != cudaSuccess) return (int)e;
-    if constexpr (PipeCfg<real, N>::enabled) {
+    if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
       const int pb = (int)PipeSmem<real, N>::bytes;
       e = cudaFuncSetAttribute(k_pipe<real, N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pb);
       if (e != cudaSuccess) return (int)e;

@@ -27,8 +27,11 @@ namespace dgrtm {
 //   F2 = 1: the volume contraction uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the FMA instructions for twice the
 //        accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 857 -> 911 us).
 template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0, TP = 0; };
+template <> struct PipeCfg<float, 2> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 2, G = 6, QS = 1, RS = 1, UG = 0, F2 = 0, TP = 0; };
+template <> struct PipeCfg<double, 2> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 2, G = 3, QS = 1, RS = 1, UG = 0, F2 = 0, TP = 0; };
 template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 2, RS = 1, UG = 0, F2 = 1, TP = 0; };
 template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = 9, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
+template <> struct PipeCfg<float, 5> { static constexpr bool enabled = true; static constexpr int TO = 8, NT = 7, G = 2, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
 template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
 
 template <typename real, int N> struct PipeSmem {
@@ -49,7 +52,10 @@ template <typename real, int N> struct PipeSmem {
   static constexpr size_t pen_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
   static constexpr size_t group_reals = C::QS * stage_reals + (size_t)(C::RS * 8 * O::Np + 4 * O::REC) * 32 + pen_reals;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
-  static constexpr size_t bytes = ops_bytes + 256 + (size_t)C::G * group_bytes;
+  // control region behind the tables: mbarriers [G][3] + table barrier, tensor-memory slot, ticket rings [G][4]
+  static constexpr size_t ring_off = ((size_t)(3 * C::G + 1) * 8 + 16 + 15) / 16 * 16;
+  static constexpr size_t ctl_bytes = (ring_off + (size_t)C::G * 16 + 127) / 128 * 128;
+  static constexpr size_t bytes = ops_bytes + ctl_bytes + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
 };
 
@@ -97,7 +103,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   int* sF = reinterpret_cast<int*>(sL + NT * NF * LL);            // [NF]
   int* sP = sF + NF;                                              // [kMaxPerm][Nfp]
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_raw + SM::ops_bytes);   // [G][3], tables
-  real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + 256);
+  real* gbase = reinterpret_cast<real*>(smem_raw + SM::ops_bytes + SM::ctl_bytes);
 
   const int tid = threadIdx.x, lane = tid & 31, wg = tid >> 5, g = wg / NT, w = wg - g * NT;
   real* grp = gbase + (size_t)g * SM::group_reals;
@@ -152,7 +158,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   // a global counter (one atomic per block, taken three turns ahead) - blocks differ in cost (levels, half-step
   // traces) and sit sorted by level, so fixed chunks would load the SMs unevenly, and a launch of a few hundred blocks
   // spreads over all SMs.  ring[j & 3] = block of the group's j-th turn (TICKETS only); bend = no block
-  int* ring = reinterpret_cast<int*>(smem_raw + SM::ops_bytes + 96) + 4 * g;
+  int* ring = reinterpret_cast<int*>(smem_raw + SM::ops_bytes + SM::ring_off) + 4 * g;
   const int bend = a.blk0 + a.nblk, ngroups = (int)gridDim.x * G;
   const int lo = a.blk0 + (int)(((long long)a.nblk * blockIdx.x) / gridDim.x);
   const int hi = a.blk0 + (int)(((long long)a.nblk * (blockIdx.x + 1)) / gridDim.x);
