@@ -32,7 +32,10 @@ template <> struct PipeCfg<double, 2> { static constexpr bool enabled = true; st
 template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 2, RS = 1, UG = 0, F2 = 1, TP = 0; };
 template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = 9, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
 template <> struct PipeCfg<float, 5> { static constexpr bool enabled = true; static constexpr int TO = 8, NT = 7, G = 2, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
+template <> struct PipeCfg<float, 6> { static constexpr bool enabled = true; static constexpr int TO = 12, NT = 7, G = 1, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
 template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
+
+template <> struct PipeCfg<double, 4> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 7, G = 1, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
 
 template <typename real, int N> struct PipeSmem {
   using O = Order<N>;
