@@ -27,12 +27,12 @@ namespace dgrtm {
 //   F2 = 1: the volume contraction uses packed fp32x2 FMAs (__ffma2_rn, sm_100): half the FMA instructions for twice the
 //        accumulators (N = 3: 395 -> 387 us on the config-4 mesh; N = 4: slower, 857 -> 911 us).
 template <typename real, int N> struct PipeCfg { static constexpr bool enabled = false; static constexpr int TO = 1, NT = 1, G = 1, QS = 1, RS = 1, UG = 1, F2 = 0, TP = 0; };
-template <> struct PipeCfg<float, 2> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 2, G = 6, QS = 1, RS = 1, UG = 0, F2 = 0, TP = 0; };
+template <> struct PipeCfg<float, 2> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 2, G = 6, QS = 1, RS = 1, UG = 0, F2 = 1, TP = 0; };
 template <> struct PipeCfg<double, 2> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 2, G = 3, QS = 1, RS = 1, UG = 0, F2 = 0, TP = 0; };
 template <> struct PipeCfg<float, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 2, RS = 1, UG = 0, F2 = 1, TP = 0; };
 template <> struct PipeCfg<float, 4> { static constexpr bool enabled = true; static constexpr int TO = 9, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
-template <> struct PipeCfg<float, 5> { static constexpr bool enabled = true; static constexpr int TO = 8, NT = 7, G = 2, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
-template <> struct PipeCfg<float, 6> { static constexpr bool enabled = true; static constexpr int TO = 12, NT = 7, G = 1, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
+template <> struct PipeCfg<float, 5> { static constexpr bool enabled = true; static constexpr int TO = 7, NT = 8, G = 2, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 1; };
+template <> struct PipeCfg<float, 6> { static constexpr bool enabled = true; static constexpr int TO = 12, NT = 7, G = 1, QS = 1, RS = 0, UG = 0, F2 = 1, TP = 1; };
 template <> struct PipeCfg<double, 3> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 4, G = 3, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
 
 template <> struct PipeCfg<double, 4> { static constexpr bool enabled = true; static constexpr int TO = 5, NT = 7, G = 1, QS = 1, RS = 0, UG = 0, F2 = 0, TP = 2; };
