@@ -140,7 +140,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     a.blk0 = md.lvl_blk0[lmin];
     a.nblk = (int)md.nblocks - a.blk0;
     if (a.nblk > 0) {
-      if (pipe && (o.nfields == 2 || !tc)) { a.sched_sel = c->sched_sel; c->sched_sel ^= 1; }   // only launches that take tickets flip the counters
+      if (pipe && (o.nfields == 2 || !tc)) { a.sched_sel = c->sched_sel; c->sched_sel ^= 1; a.reverse = L == 1 ? (int)(m & 1) : 0; }   // only launches that take tickets flip the counters
       if (o.nfields == 2) DG_LAUNCH(c, KC_STEP_IMAGE, pipe ? c->kt->pipe2(a, c->stream) : c->kt->step2(a, c->stream));
       else DG_LAUNCH(c, KC_STEP, tc ? c->kt->tc(a, c->stream) : (pipe ? c->kt->pipe(a, c->stream) : c->kt->step(a, c->stream)));
     }

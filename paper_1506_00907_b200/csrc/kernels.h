@@ -132,6 +132,8 @@ struct StepArgs {
   const unsigned char* blkflag;   // per block: bit 0 = some element has a finer face neighbour
   unsigned* sched; int sched_sel;   // two ticket counters of the pipelined kernel's work distribution; this launch uses [sched_sel]
   int sched_mode;                   // 0: fixed contiguous chunks per CTA; 1: interleaved start, then blocks by ticket
+  int reverse;                      // fixed chunks walked from their end: alternates from launch to launch, so a step starts
+                                    // with the blocks the previous step left in L2 (matters when the mesh nearly fits it)
   const void* ext;           // prescribed exterior states or null
   double dir;
   // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale

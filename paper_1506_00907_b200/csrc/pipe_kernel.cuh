@@ -176,7 +176,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
   const int nitems = nmine > 0 ? nmine * NFLD : 0;
   auto item_block = [&](int i) {
     if constexpr (TICKETS) return ring[(i / NFLD) & 3];
-    else return lo + g + (i / NFLD) * G;
+    else return a.reverse ? hi - 1 - g - (i / NFLD) * G : lo + g + (i / NFLD) * G;
   };
   auto has_item = [&](int i) {                                    // the group has an i-th item
     if constexpr (TICKETS) return ring[(i / NFLD) & 3] < bend;
