@@ -416,6 +416,28 @@ def test_full_size_short_run(name, nsteps):
         g.close()
 
 
+@pytest.mark.parametrize("N,nsteps,levels", [(2, 4, 1), (5, 2, 1), (6, 1, 1), (4, 2, 1), (2, 1, 3)])
+def test_full_size_short_run_other_orders(N, nsteps, levels):
+    """The pipelined kernel at the orders it serves besides N = 3 (k_pipe<float,2 / 5 / 6>, k_pipe<double,2 / 4>; fp64 at N = 5,
+    6: k_step) on the GPU-filling config-2 mesh (98 304 tetrahedra = 3 072 blocks; config-3 mesh with three levels for the
+    ticket mode): a few steps from a random state against the live oracle, every element compared."""
+    cfg = make_config("cfg2_two_layer" if levels == 1 else "cfg3_lts", N=N)
+    cfg["receivers"] = None
+    o = make_oracle(cfg)
+    q0 = random_state(o.K, o.Np, 13 + N)
+    F = o.new_field(q0)
+    o.run_mrab([F], nsteps, 0.0, 1, source_on=(True,))
+    for precision in (32, 64):
+        g = make_gpu(cfg, precision)
+        assert g.K == (98304 if levels == 1 else 331776)
+        g.dg_set_state(q0)
+        g.dg_step(nsteps)
+        qg = g.dg_get_fields()
+        assert rel_l2(qg, F.q) < TOL[precision]
+        assert per_element_max(qg, F.q) < 20 * TOL[precision]
+        g.close()
+
+
 def test_full_size_rtm_two_steps():
     """Config 4 at full size (786 432 tetrahedra, 32 768 stored boundary faces): two forward steps with trace capture and
     receiver recording, two backward steps of both wavefields with replay, injection and imaging, against the live
