@@ -246,15 +246,16 @@ def profile_kernels(g, T, reps, elems_per_global_step, Np, Nfp, rs, peak, peak_s
 
 def run_e2e(g, torch, T, K, q0, device):
     """Same metric through the C ABI with host buffers: set_state(host) -> step -> get_fields(host)."""
+    q = np.empty_like(q0)                       # the caller's result buffer, reused from step to step
     g.dg_set_state(q0)
     g.dg_step(T)
-    g.dg_get_fields()
+    g.dg_get_fields(out=q)
     torch.cuda.synchronize(device)
     t0 = time.perf_counter()
     for _ in range(K):
         g.dg_set_state(q0)
         g.dg_step(T)
-        q = g.dg_get_fields()
+        g.dg_get_fields(out=q)
     torch.cuda.synchronize(device)
     sec = time.perf_counter() - t0
     return sec, q

@@ -362,8 +362,10 @@ class DG:
         self._ck(_lib.dg_get_receivers(self._h, _ptr(k, _pi32), _ptr(rows, _pd), _ptr(w, _pd)))
         return k, rows, w
 
-    def dg_get_fields(self):
-        q = np.empty((self.K, 4, self.Np))
+    def dg_get_fields(self, out=None):
+        """q[K][4][Np] in user order; `out` = a C-contiguous float64 array of that shape to fill instead of a new one."""
+        q = np.empty((self.K, 4, self.Np)) if out is None else out
+        assert q.shape == (self.K, 4, self.Np) and q.dtype == np.float64 and q.flags.c_contiguous
         self._ck(_lib.dg_get_fields(self._h, _ptr(q, _pd)))
         return q
 

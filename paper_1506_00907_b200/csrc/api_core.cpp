@@ -171,21 +171,31 @@ template <typename real> void unpack_fields(const dg_ctx* c, double* q, const re
 }
 }  // namespace
 
+char* host_stage(dg_ctx* c, size_t bytes) {
+  if (bytes > c->stage_bytes) {
+    if (c->stage_host) cudaFreeHost(c->stage_host);
+    c->stage_host = nullptr; c->stage_bytes = 0;
+    cuda_check(cudaHostAlloc(reinterpret_cast<void**>(&c->stage_host), bytes, cudaHostAllocDefault), "cudaHostAlloc (staging)");
+    c->stage_bytes = bytes;
+  }
+  return c->stage_host;
+}
+
 void fields_to_device(dg_ctx* c, char* dq, const double* q) {
-  const size_t n = (size_t)c->model.nslots * 4 * c->Np;
-  std::vector<char> tmp(n * c->rs);
-  if (c->precision == 64) pack_fields(c, reinterpret_cast<double*>(tmp.data()), q);
-  else pack_fields(c, reinterpret_cast<float*>(tmp.data()), q);
-  upload_raw(c, dq, tmp.data(), tmp.size());
+  const size_t nbytes = (size_t)c->model.nslots * 4 * c->Np * c->rs;
+  char* tmp = host_stage(c, nbytes);            // pinned: the copy runs at link speed, no hidden staging
+  if (c->precision == 64) pack_fields(c, reinterpret_cast<double*>(tmp), q);
+  else pack_fields(c, reinterpret_cast<float*>(tmp), q);
+  upload_raw(c, dq, tmp, nbytes);
 }
 
 void fields_from_device(dg_ctx* c, double* q, const char* dq) {
-  const size_t n = (size_t)c->model.nslots * 4 * c->Np;
-  std::vector<char> tmp(n * c->rs);
-  cuda_check(cudaMemcpyAsync(tmp.data(), dq, tmp.size(), cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
+  const size_t nbytes = (size_t)c->model.nslots * 4 * c->Np * c->rs;
+  char* tmp = host_stage(c, nbytes);
+  cuda_check(cudaMemcpyAsync(tmp, dq, nbytes, cudaMemcpyDeviceToHost, c->stream), "cudaMemcpyAsync D2H");
   sync_stream(c);
-  if (c->precision == 64) unpack_fields(c, q, reinterpret_cast<const double*>(tmp.data()));
-  else unpack_fields(c, q, reinterpret_cast<const float*>(tmp.data()));
+  if (c->precision == 64) unpack_fields(c, q, reinterpret_cast<const double*>(tmp));
+  else unpack_fields(c, q, reinterpret_cast<const float*>(tmp));
 }
 
 // user order I[K][Np] <- device [block][Np][32], one threaded pass from the device precision
@@ -297,6 +307,7 @@ dg_ctx::~dg_ctx() {
     for (cudaEvent_t e : ev_copy[l]) cudaEventDestroy(e);
   }
   if (copy_stream) cudaStreamDestroy(copy_stream);
+  if (stage_host) cudaFreeHost(stage_host);
 }
 extern "C" {
 

@@ -172,6 +172,9 @@ struct dg_ctx {
   std::vector<cudaEvent_t> ev_step[dgrtm::kMaxLevels];   // bound stream: the launch that wrote / read the slot
   std::vector<cudaEvent_t> ev_copy[dgrtm::kMaxLevels];   // copy stream: the slot's last transfer
 
+  // pinned host staging for the field transfers of dg_set_state / dg_get_fields / rtm_get_fields (grown on demand)
+  char* stage_host = nullptr;
+  size_t stage_bytes = 0;
   int64_t launches = 0;
   // per-kernel timing (dg_set_profiling): one CUDA event pair per launch on the bound stream
   bool prof = false;
@@ -195,6 +198,7 @@ void sync_stream(dg_ctx* c);
 // user order q[K][4][Np]  <->  device [block][4Np][32]
 void fields_to_device(dg_ctx* c, char* dq, const double* q);
 void fields_from_device(dg_ctx* c, double* q, const char* dq);
+char* host_stage(dg_ctx* c, size_t bytes);   // the ctx's pinned staging buffer, at least `bytes` large
 void image_from_device(dg_ctx* c, double* I, const char* dimg);   // user order I[K][Np] <- device [block][Np][32]
 void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
 void normalize_traces(dg_ctx* c, Field& F);
