@@ -123,22 +123,25 @@ void copy_data(dg_ctx* c, double* host, const double* host_in, int64_t ncol) {
   const int64_t nsamp = (int64_t)c->hist_nsteps * c->nlocal + 1;
   const size_t rs = c->rs;
   if (c->nr == 0) return;
+  const size_t n = (size_t)c->nr * ncol;
+  char* tmp = host_stage(c, n * rs);             // pinned staging, conversions on host threads
+  const bool f64 = c->precision == 64;
   if (host_in) {
-    std::vector<char> tmp((size_t)c->nr * ncol * rs);
-    for (size_t i = 0; i < (size_t)c->nr * ncol; ++i) {
-      if (c->precision == 64) ((double*)tmp.data())[i] = host_in[i];
-      else ((float*)tmp.data())[i] = (float)host_in[i];
-    }
-    cuda_check(cudaMemcpy2DAsync(c->d_data, nsamp * rs, tmp.data(), ncol * rs, ncol * rs, c->nr,
+    parallel_range(n, [&](size_t a, size_t b) {
+      if (f64) for (size_t i = a; i < b; ++i) ((double*)tmp)[i] = host_in[i];
+      else for (size_t i = a; i < b; ++i) ((float*)tmp)[i] = (float)host_in[i];
+    });
+    cuda_check(cudaMemcpy2DAsync(c->d_data, nsamp * rs, tmp, ncol * rs, ncol * rs, c->nr,
                                  cudaMemcpyHostToDevice, c->stream), "cudaMemcpy2DAsync data H2D");
     sync_stream(c);
   } else {
-    std::vector<char> tmp((size_t)c->nr * ncol * rs);
-    cuda_check(cudaMemcpy2DAsync(tmp.data(), ncol * rs, c->d_data, nsamp * rs, ncol * rs, c->nr,
+    cuda_check(cudaMemcpy2DAsync(tmp, ncol * rs, c->d_data, nsamp * rs, ncol * rs, c->nr,
                                  cudaMemcpyDeviceToHost, c->stream), "cudaMemcpy2DAsync data D2H");
     sync_stream(c);
-    for (size_t i = 0; i < (size_t)c->nr * ncol; ++i)
-      host[i] = c->precision == 64 ? ((double*)tmp.data())[i] : (double)((float*)tmp.data())[i];
+    parallel_range(n, [&](size_t a, size_t b) {
+      if (f64) for (size_t i = a; i < b; ++i) host[i] = ((const double*)tmp)[i];
+      else for (size_t i = a; i < b; ++i) host[i] = (double)((const float*)tmp)[i];
+    });
   }
 }
 

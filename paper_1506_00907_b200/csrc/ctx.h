@@ -2,10 +2,12 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
 #include <cstring>
 #include <stdexcept>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/dgrtm.h"
@@ -198,6 +200,21 @@ void sync_stream(dg_ctx* c);
 // user order q[K][4][Np]  <->  device [block][4Np][32]
 void fields_to_device(dg_ctx* c, char* dq, const double* q);
 void fields_from_device(dg_ctx* c, double* q, const char* dq);
+// [0, n) split over host threads (conversions between the caller's doubles and the device precision)
+template <typename F> void parallel_range(size_t n, F body) {
+  unsigned nt = std::thread::hardware_concurrency();
+  nt = nt == 0 ? 1 : (nt > 16 ? 16 : nt);
+  if (n < (size_t)1 << 16) nt = 1;
+  if (nt == 1) { body((size_t)0, n); return; }
+  std::vector<std::thread> th;
+  const size_t per = (n + nt - 1) / nt;
+  for (unsigned t = 0; t < nt; ++t) {
+    const size_t a = t * per, b = std::min(n, a + per);
+    if (a >= b) break;
+    th.emplace_back([=] { body(a, b); });
+  }
+  for (auto& x : th) x.join();
+}
 char* host_stage(dg_ctx* c, size_t bytes);   // the ctx's pinned staging buffer, at least `bytes` large
 void image_from_device(dg_ctx* c, double* I, const char* dimg);   // user order I[K][Np] <- device [block][Np][32]
 void refresh_traces(dg_ctx* c, Field& F);   // qf := traces of q, all levels
