@@ -438,6 +438,27 @@ def test_full_size_short_run_other_orders(N, nsteps, levels):
         g.close()
 
 
+@pytest.mark.parametrize("name", ["cfg2_two_layer", "cfg3_lts", "cfg4_rtm"])
+def test_full_size_full_length_fp32_against_fp64(name):
+    """BASELINE.json configs 2, 3, 4 at FULL size and FULL length (1000 steps; 500 global steps of three levels at N = 4; 2000
+    steps), in the launch configuration bench.py times: the oracle cannot run these, so the fp32 path is compared with the
+    fp64 path of the library, which is itself pinned to the oracle at full length on the 41 472-element meshes
+    (tests/test_gpu_goldens.py) and at full size over a few steps (test_full_size_short_run).  north_star: relative L2
+    <= 1e-5 in fp32 after the stated step counts."""
+    cfg = make_config(name)
+    cfg["receivers"] = None
+    q = {}
+    for precision in (64, 32):
+        g = make_gpu(cfg, precision)
+        g.dg_step(cfg["nsteps"])
+        q[precision] = g.dg_get_fields()
+        g.close()
+    assert np.linalg.norm(q[64]) > 0
+    err = rel_l2(q[32], q[64])
+    assert err < TOL[32], err
+    assert per_element_max(q[32], q[64]) < 20 * TOL[32]
+
+
 def test_full_size_rtm_two_steps():
     """Config 4 at full size (786 432 tetrahedra, 32 768 stored boundary faces): two forward steps with trace capture and
     receiver recording, two backward steps of both wavefields with replay, injection and imaging, against the live
