@@ -100,3 +100,26 @@ def test_decomposed_run_matches_the_oracle(N, precision, nparts):
     q1 = g.dg_get_fields()
     g.close()
     assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
+
+
+@pytest.mark.gpu
+def test_halo_and_spill_calls_reject_bad_arguments():
+    """Error behaviour stated in include/dgrtm.h: wrong arguments come back as error codes (DGError), nothing aborts."""
+    import paper_1506_00907_b200 as pk
+    cfg = _cfg(hexes=(3, 3, 2))
+    g = make_gpu(cfg, 32)                                            # absorbing faces only: none is DG_BC_PRESCRIBED
+    Nfp = g.Nfp
+    with pytest.raises(pk.DGError):
+        g.dg_set_halo(0, np.array([0]), np.array([0]), np.zeros((1, Nfp), dtype=np.int32))      # not a prescribed face
+    with pytest.raises(pk.DGError):
+        g.dg_set_halo(9, np.array([0]), np.array([0]), np.zeros((1, Nfp), dtype=np.int32))      # set out of range
+    with pytest.raises(pk.DGError):
+        g.dg_halo_pull(0, 0)                                         # NULL source
+    with pytest.raises(pk.DGError):
+        g.rtm_set_trace_spill(1 << 20, 4096, 1)                      # window < 2
+    g.close()
+    cfg3 = make_config("cfg3_lts", hexes=(4, 4, 6), N=2)
+    g = make_gpu(cfg3, 32)
+    with pytest.raises(pk.DGError):
+        g.dg_get_trace_device()                                      # the halo exchange is single-rate
+    g.close()
