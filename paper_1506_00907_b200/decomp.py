@@ -9,9 +9,12 @@ fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_hal
 
 The paper partitions with METIS, cell weights 2^(l-1) and keeps the finest cells off the cuts
 (PAPER.md:387); METIS is not in this container: `partition_elements` is a weighted coordinate bisection that takes the same
-weights.  Here all sub-domains live in one process (on one GPU their launches are ordered by the shared stream); with one
-process per GPU the source pointer of `dg_halo_pull` is a peer mapping of the neighbour's trace buffer and the loads
-cross NVLink - that launch mode needs more than the one GPU this pool grants and is not exercised.
+weights.  `Decomposition` keeps all sub-domains in one process (on one GPU their launches are ordered by the shared stream).
+`RankDecomposition` is the one-process-per-sub-domain mode (one rank of torch.distributed = one sub-domain = one GPU): the
+ranks exchange CUDA IPC handles of their workspaces once, after which the source pointer of `dg_halo_pull` is the peer
+mapping of the neighbour's trace buffer - the loads of k_halo cross NVLink (or stay on the device when the ranks share a
+GPU, which is how tests/test_decomp.py exercises it: this pool grants one GPU).  The ranks step in lock-step through a
+host barrier per time step (no kernel waits on another).
 """
 import numpy as np
 
@@ -48,7 +51,9 @@ def partition_elements(EToV, VX, nparts, weights=None):
 class Decomposition:
     """The sub-domains of one mesh as DG contexts with their halo tables.  Global arrays in, global arrays out."""
 
-    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15):
+    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15, only=None):
+        """only = p: bind / step sub-domain p alone (the others exist on the host for their slot tables)."""
+        self.only = only
         EToV = np.ascontiguousarray(EToV, dtype=np.int32)
         self.K, self.part = EToV.shape[0], np.asarray(part, dtype=np.int32)
         self.nparts = int(self.part.max()) + 1
@@ -104,8 +109,12 @@ class Decomposition:
             self.sets.append(sets)
 
     # ---- memory, set-up
+    def mine(self):
+        return range(self.nparts) if self.only is None else (self.only,)
+
     def bind_torch(self, device="cuda:0"):
-        for p, s in enumerate(self.sub):
+        for p in self.mine():
+            s = self.sub[p]
             s.bind_torch(device)
             s.dg_set_dt(self.dt)                                      # the global stable step, not the sub-domain's own
             for i, (q, bnd, rec, pos) in enumerate(self.sets[p]):
@@ -148,3 +157,64 @@ class Decomposition:
     def close(self):
         for s in self.sub:
             s.close()
+
+
+class RankDecomposition(Decomposition):
+    """One sub-domain per torch.distributed rank.  Every rank builds the host side of all sub-domains (their slot tables
+    are needed for the halo tables), binds its own, and maps the workspaces of its neighbours through CUDA IPC; the
+    trace buffer of a neighbour is then addressed as (mapped workspace base + the offset that neighbour reports)."""
+
+    def __init__(self, dist, *args, **kw):
+        self.dist, self.rank = dist, dist.get_rank()
+        super().__init__(*args, only=self.rank, **kw)
+        assert self.nparts == dist.get_world_size(), "one sub-domain per rank"
+
+    def bind_torch(self, device="cuda:0"):
+        import torch
+        from torch.multiprocessing.reductions import reduce_tensor
+        super().bind_torch(device)
+        me = self.sub[self.rank]
+        self._device = device
+        handles = [None] * self.nparts
+        self.dist.all_gather_object(handles, reduce_tensor(me._ws))       # (rebuild function, arguments) per rank
+        self._peer = {}
+        for q, _, _, _ in self.sets[self.rank]:
+            fn, a = handles[q]
+            self._peer[q] = fn(*a)                                        # the neighbour's workspace tensor, mapped here
+        self.dist.barrier()
+
+    def _trace_offsets(self):
+        """Offset of every rank's current trace buffer inside its workspace tensor (a host-side all-gather)."""
+        me = self.sub[self.rank]
+        off = me.dg_get_trace_device()[0] - me._ws.data_ptr()
+        offs = [None] * self.nparts
+        self.dist.all_gather_object(offs, int(off))
+        return offs
+
+    def dg_step(self, nsteps):
+        import torch
+        me = self.sub[self.rank]
+        for _ in range(int(nsteps)):
+            offs = self._trace_offsets()            # also orders this step after every rank's previous step (see below)
+            for i, (q, _, _, _) in enumerate(self.sets[self.rank]):
+                me.dg_halo_pull(i, self._peer[q].data_ptr() + offs[q])
+            torch.cuda.synchronize(self._device)    # my fetches have read the neighbours' traces ...
+            self.dist.barrier()                     # ... on every rank, before anybody's step overwrites them
+            me.dg_step(1)
+            torch.cuda.synchronize(self._device)    # my new traces are complete before the next all-gather returns
+
+    def dg_set_state(self, q, t0=0.0):
+        self.sub[self.rank].dg_set_state(q[self.elems[self.rank]], t0)
+
+    def dg_get_fields(self):
+        """Global field on every rank (host all-gather of the sub-domain fields)."""
+        mine = self.sub[self.rank].dg_get_fields()
+        parts = [None] * self.nparts
+        self.dist.all_gather_object(parts, mine)
+        q = np.empty((self.K, 4, self.Np))
+        for p in range(self.nparts):
+            q[self.elems[p]] = parts[p]
+        return q
+
+    def launch_count(self):
+        return self.sub[self.rank].dg_get_launch_count()

@@ -123,3 +123,27 @@ def test_halo_and_spill_calls_reject_bad_arguments():
     with pytest.raises(pk.DGError):
         g.dg_get_trace_device()                                      # the halo exchange is single-rate
     g.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("N,precision,world", [(3, 64, 2), (3, 32, 3)])
+def test_one_process_per_sub_domain(N, precision, world, tmp_path):
+    """RankDecomposition: one process per sub-domain (gloo for the host side, CUDA IPC mappings of the neighbours'
+    workspaces as the source of k_halo), all on cuda:0 here.  Same result as the single-domain run of the library."""
+    import socket
+    import torch.multiprocessing as mp
+    import decomp_worker
+    nsteps, hexes = 60, (6, 5, 4)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "q.npy")
+    mp.spawn(decomp_worker.run, args=(world, port, N, precision, nsteps, hexes, out), nprocs=world, join=True)
+    q = np.load(out)
+    cfg = _cfg(hexes=hexes, N=N)
+    g = make_gpu(cfg, precision)
+    g.dg_step(nsteps)
+    q1 = g.dg_get_fields()
+    g.close()
+    assert np.linalg.norm(q1) > 0
+    assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
