@@ -32,3 +32,59 @@ def run(rank, world, port, N, precision, nsteps, hexes, out_path):
     dist.barrier()
     dd.close()
     dist.destroy_process_group()
+
+
+def check_plan(rank, world, port, N, hexes, out_path):
+    """CPU (gloo) check of the one-process-per-sub-domain plan: every rank asks each neighbour - which answers from its OWN
+    sub-domain only - for the physical coordinates of the trace-record entries it is going to read, and compares them
+    with the coordinates of its own halo face nodes."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    here = os.path.dirname(os.path.abspath(__file__))
+    sys.path.insert(0, os.path.dirname(here))
+    from workloads import make_config
+    from paper_1506_00907_b200.decomp import RankDecomposition, partition_elements
+    cfg = make_config("cfg2_two_layer", hexes=hexes, N=N)
+    etov, vx = cfg["EToV"], cfg["VX"]
+    part = partition_elements(etov, vx, world)
+    dd = RankDecomposition(dist, N, 64, etov, vx, cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"])
+    me = dd.sub[rank]
+
+    def node_xyz(elems_global):
+        r, s, t = me.dg_get_nodes()
+        L = np.stack([-(1 + r + s + t) / 2, (1 + r) / 2, (1 + s) / 2, (1 + t) / 2], axis=1)
+        return np.einsum("nv,kvd->knd", L, vx[etov[elems_global]])
+
+    Fmask = me.dg_get_operators()[4]
+    mine_xyz = node_xyz(dd.elems[rank])                               # [Kp][Np][3] of MY elements
+    slot_to_elem = np.argsort(me.dg_get_slots())                      # my slots are a permutation of 0..Kp-1 plus padding
+    slots = me.dg_get_slots()
+    lookup = {int(sl): k for k, sl in enumerate(slots)}
+    requests = [None] * world
+    dist.all_gather_object(requests, {q: (rec, pos) for q, _, rec, pos in dd.sets[rank]})
+    answers = {}
+    for p in range(world):                                            # what rank p wants to read from MY buffer
+        if p != rank and rank in requests[p]:
+            rec, pos = requests[p][rank]
+            k = np.array([lookup[int(x)] for x in rec // 4])
+            f = (rec % 4).astype(int)
+            answers[p] = np.stack([mine_xyz[k[h]][Fmask[f[h]]][pos[h]] for h in range(len(rec))])
+    replies = [None] * world
+    dist.all_gather_object(replies, answers)
+    bk, bf, _ = me.dg_get_boundary_faces()
+    worst, n = 0.0, 0
+    for q, bnd, rec, pos in dd.sets[rank]:
+        theirs = replies[q][rank]
+        for h in range(len(bnd)):
+            own = mine_xyz[bk[bnd[h]]][Fmask[bf[bnd[h]]]]
+            worst = max(worst, float(np.abs(own - theirs[h]).max()))
+            n += 1
+    res = [None] * world
+    dist.all_gather_object(res, (worst, n))
+    if rank == 0:
+        np.save(out_path, np.array(res))
+    dist.barrier()
+    dd.close()
+    dist.destroy_process_group()

@@ -147,3 +147,20 @@ def test_one_process_per_sub_domain(N, precision, world, tmp_path):
     g.close()
     assert np.linalg.norm(q1) > 0
     assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_rank_decomposition_plan_gloo(world, tmp_path):
+    """The N > 1 path on the CPU (gloo, world size 2 and 3): every rank's halo requests, answered by the neighbour from its
+    own sub-domain alone, are the coordinates of the requester's halo face nodes (tests/decomp_worker.py::check_plan)."""
+    import socket
+    import torch.multiprocessing as mp
+    import decomp_worker
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "plan.npy")
+    mp.spawn(decomp_worker.check_plan, args=(world, port, 3, (5, 4, 3), out), nprocs=world, join=True)
+    res = np.load(out)
+    assert res.shape == (world, 2) and res[:, 1].min() > 0           # every rank has halo faces
+    assert res[:, 0].max() < 1e-12
