@@ -105,6 +105,18 @@ int dg_set_state(dg_ctx* ctx, const double* q, double t0);
  * the update (18) of the levels that land on the step end and the half-step traces (19) of their
  * not-updated coarse neighbours (Alg. 1, Alg. 4).  Asynchronous on the stream. */
 int dg_step(dg_ctx* ctx, int nsteps);
+/* dg_step under DG_INTEGRATOR_LSERK4 (reading Q8) for callers that cannot allocate (CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same time loop, but the 2N-storage residual of the stage kernel lives in a
+ * file-scope device array of the library instead of the workspace, and the call makes no cudaMalloc / cudaFree and uses no
+ * allocating library routine.  Inputs and outputs are the context's bound workspace as for dg_step.  The array is
+ * dg_static_scratch_bytes = 8 MiB on every GPU that loads the library, until the process exits; a state whose field
+ * array [nslots][4 Np] is larger is rejected with DG_ERR_NOMEM (use dg_step).  DG_ERR_STATE unless the integrator is
+ * LSERK4 and dg_set_profiling is off (profiling creates events).  The array is shared by all calls and contexts on a GPU
+ * and keeps the last call's contents: every call clears what it uses first; calls whose kernels overlap on the GPU
+ * (different streams) race on it - serialise them.  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress): make one call before capturing a graph. */
+int dg_step_lserk4_static(dg_ctx* ctx, int nsteps);
+int dg_static_scratch_bytes(size_t* n);
 /* Prescribed-exterior faces (DG_BC_PRESCRIBED; plane-wave tests): exterior traces (p+, n.v+ with the
  * owner's outward normal) ext[nbnd][Nfp][2] in boundary-face-list order, used by every following
  * right-hand side until replaced.  Entries of faces of another type are ignored. */

@@ -52,6 +52,8 @@ SIGNATURES = {
     "dg_set_state": (_i, [_vp, _pd, _d]),
     "dg_step": (_i, [_vp, _i]),
     "dg_set_exterior": (_i, [_vp, _pd]),
+    "dg_step_lserk4_static": (_i, [_vp, _i]),
+    "dg_static_scratch_bytes": (_i, [C.POINTER(_sz)]),
     "dg_set_exterior_impedance": (_i, [_vp, _pd]),
     "dg_get_slots": (_i, [_vp, _pi64]),
     "dg_get_trace_device": (_i, [_vp, C.POINTER(_vp), C.POINTER(_sz)]),
@@ -104,6 +106,13 @@ class DGError(RuntimeError):
 
 def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def dg_static_scratch_bytes():
+    n = _sz()
+    rc = _lib.dg_static_scratch_bytes(C.byref(n))
+    assert rc == DG_OK
+    return n.value
 
 
 def _ptr(a, typ):
@@ -195,6 +204,10 @@ class DG:
 
     def dg_step(self, nsteps):
         self._ck(_lib.dg_step(self._h, int(nsteps)))
+
+    def dg_step_lserk4_static(self, nsteps):
+        """LSERK4 steps with the stage residual in the library's static device array (no allocation; <= 8 MiB of state)."""
+        self._ck(_lib.dg_step_lserk4_static(self._h, int(nsteps)))
 
     def dg_set_exterior(self, ext):
         ext = _f64(ext)
