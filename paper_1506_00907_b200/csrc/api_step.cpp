@@ -80,7 +80,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.dir = (double)dir;
   a.ops = c->ops; a.ops.D3T = c->d_D3P; a.ops.LIFTT = c->d_LTP;
   a.ops2_D3Q = c->d_D3Q; a.ops2_LTQ = c->d_LTQ;
-  const bool pipe = c->use_pipe && c->kt->pipe != nullptr;
+  const bool pipe = c->use_pipe && c->kt->pipe != nullptr && c->ops.nperm <= 8;   // (a triangle has 6; the pipelined kernel's gather table holds 8)
   const bool tc = c->use_tc && c->kt->tc != nullptr && o.nfields == 1;
   a.image = c->image; a.img_scratch = c->scratch; a.characteristic = (o.imaging & 1) != 0;
   a.trapezoid = (o.imaging & 2) != 0;

@@ -174,6 +174,7 @@ template <typename real> KernelTable make_table(int precision) {
     t.tc = Launch<real>::tc; t.tc_K1 = TcSmem<N>::K1; t.tc_K2 = TcSmem<N>::K2; t.tc_NN = TcSmem<N>::NN;
     t.tc_blob_bytes = TcSmem<N>::ops_bytes;
   }
+  static_assert(!PipeCfg<real, N>::enabled || PipeSmem<real, N>::fits, "an enabled pipelined configuration must fit the 227 KB of shared memory");
   if constexpr (PipeCfg<real, N>::enabled && PipeSmem<real, N>::fits) {
     t.pipe = Launch<real>::pipe; t.pipe2 = Launch<real>::pipe2;
     t.pipe_TO = PipeCfg<real, N>::TO; t.pipe_NT = PipeCfg<real, N>::NT;

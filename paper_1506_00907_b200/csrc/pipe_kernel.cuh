@@ -52,11 +52,22 @@ template <typename real, int N> struct PipeSmem {
   static constexpr size_t stage_reals = (size_t)(4 * O::Np + DG_NGEO) * 32;
   // penalties: [face][Pp | Pv][ceil(Nfp / VW)][lane][VW] (one vector load = VW face nodes of my element)
   static constexpr int PV = (O::Nfp + VW - 1) / VW;               // vectors per face and penalty kind
-  static constexpr size_t pen_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
+  // trace staging (after the update the penalties are dead): [element-lane][4 REC reals] = the block's records exactly as
+  // they lie in global memory, the element stride padded to an ODD number SU of 16-byte units (vector stores of 8
+  // consecutive lanes then cover all banks once)
+  static constexpr int UE = 4 * O::REC * (int)sizeof(real) / 16;  // 16-byte units of one element's four records
+  static constexpr int SU = UE | 1;
+  static constexpr size_t stg_reals = (size_t)32 * SU * 16 / sizeof(real);
+  static constexpr size_t pen0_reals = (size_t)(8 * PV * VW > 2 * O::NF ? 8 * PV * VW : 2 * O::NF) * 32;
+  static constexpr size_t pen_reals = pen0_reals > stg_reals ? pen0_reals : stg_reals;
   static constexpr size_t group_reals = C::QS * stage_reals + (size_t)(C::RS * 8 * O::Np + 4 * O::REC) * 32 + pen_reals;
   static constexpr size_t group_bytes = group_reals * sizeof(real);
   // control region behind the tables: mbarriers [G][3] + table barrier, tensor-memory slot, ticket rings [G][4]
   static constexpr size_t ring_off = ((size_t)(3 * C::G + 1) * 8 + 16 + 15) / 16 * 16;
+  // the gather table of the trace phase, qtab[perm][face][pos] = offset in q of the own face node whose value goes to
+  // position pos of the record the neighbour reads, is built in the prologue OVER the permutation table of the blob
+  // (kMaxPerm x Nfp ints = kPerm x 4 x Nfp: a triangle's node set has at most 6 such permutations)
+  static constexpr int kPerm = UpdSmem<N>::kMaxPerm / 4;
   static constexpr size_t ctl_bytes = (ring_off + (size_t)C::G * 16 + 127) / 128 * 128;
   static constexpr size_t bytes = ops_bytes + ctl_bytes + (size_t)C::G * group_bytes;
   static constexpr bool fits = bytes <= 227 * 1024;
@@ -229,12 +240,12 @@ k_pipe(const __grid_constant__ StepArgs a) {
   };
   // write-out pieces of this warp (it = w + k NT): staging offset of piece P = it*32 + lane (rows VS (P % NV) .. of
   // element-lane P / NV, column rotated by the piece index)
-  constexpr int WO_VS = 16 / (int)sizeof(real), WO_NV = 4 * REC / WO_VS, WOK = (WO_NV + NT - 1) / NT;
-  int wo_src[WOK];
+  constexpr int WO_NV = SM::UE, WOK = (WO_NV + NT - 1) / NT;
+  int wo_src[WOK];                                                // byte offset of the piece in the staging
 #pragma unroll
   for (int k = 0; k < WOK; ++k) {
     const int P = (w + k * NT) * 32 + lane, el = P / WO_NV, o4 = P - el * WO_NV;
-    wo_src[k] = o4 * WO_VS * 32 + ((el + o4) & 31);
+    wo_src[k] = (el * SM::SU + o4) * 16;
   }
   // piece P = it*32 + lane of a face's 32 records belongs to element-lane P / NP, offset (P % NP) CPW in its record
   int gth_r[REC / CPW], gth_v[REC / CPW];
@@ -287,6 +298,26 @@ k_pipe(const __grid_constant__ StepArgs a) {
   load_codes(0, codeA);
   load_codes(1, codeB);
   mbar_wait(tabbar, 0);
+  int* sQT = sP;                                                  // [kPerm][4][Nfp], built in place over the permutation table
+  {
+    constexpr int EPT = (SM::kPerm * 4 * Nfp + NTHREADS - 1) / NTHREADS;   // entries per thread
+    const int np = a.ops.nperm < SM::kPerm ? a.ops.nperm : SM::kPerm;
+    int dst_i[EPT], val[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+      const int x = tid + e * NTHREADS;
+      dst_i[e] = -1;
+      if (x < np * 4 * Nfp) {
+        const int pf = x / Nfp, i2 = x - pf * Nfp, pid = pf >> 2, f = pf & 3;
+        dst_i[e] = pf * Nfp + sP[pid * Nfp + i2];
+        val[e] = sF[f * Nfp + i2] * 32;
+      }
+    }
+    __syncthreads();                                              // every entry of the permutation table has been read
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) if (dst_i[e] >= 0) sQT[dst_i[e]] = val[e];
+    __syncthreads();
+  }
   int fofs[FPW][Nfp];                                             // own-trace offsets of this warp's faces in Q
 #pragma unroll
   for (int k = 0; k < FPW; ++k)
@@ -695,21 +726,38 @@ k_pipe(const __grid_constant__ StepArgs a) {
           }
       }
       if (pass == 1) group_sync<NT>(g);         // Q holds the values of this pass; pen is free
+      // gather formulation: position r of the record (the READER's node order) takes the own face node qtab[perm][f][r];
+      // the record is built in registers in its final order and stored with vector stores into the staging, which has
+      // the block's global layout [element-lane][face][p | n.v] (element stride padded, PipeSmem)
+      char* stg = reinterpret_cast<char*>(pen);
 #pragma unroll
       for (int k = 0; k < FPW; ++k) {
         const int f = w + k * NT;
         if (f < 4) {
           const real nx = geo[(GEO_FACE + 5 * f + 0) * 32], ny = geo[(GEO_FACE + 5 * f + 1) * 32], nz = geo[(GEO_FACE + 5 * f + 2) * 32];
-          const int* prow = sP + ((wp >> (8 * f)) & 255) * Nfp;
-          // staging [row][lane] with the lane rotated by row / VS: conflict-free for these stores (rows of one
-          // instruction lie within one face) and for the piece-wise reads of the write-out below
-          constexpr int VS = 16 / (int)sizeof(real);
+          const int* qrow = sQT + (((wp >> (8 * f)) & 255) * 4 + f) * Nfp;
+          const real* Ql = Q + lane;
+          constexpr int SWB = (REC * (int)sizeof(real)) % 16 == 0 ? 16 : 8, SW = SWB / (int)sizeof(real);   // store width
+          using VS_t = typename VecT<real, SW>::T;
+          VS_t* out = reinterpret_cast<VS_t*>(stg + (size_t)lane * (SM::SU * 16) + (size_t)f * (REC * sizeof(real)));
+          constexpr bool QREG = Nfp >= 10;                         // keep the offsets in registers (each is used for p and for n.v)
+          int qo[QREG ? Nfp : 1];                                   // offsets of the record's nodes, in the reader's order
+          if constexpr (QREG) {
 #pragma unroll
-          for (int i2 = 0; i2 < Nfp; ++i2) {
-            const int o = fofs[k][i2], pos = prow[i2];
-            const int rp = f * REC + pos, rv = rp + Nfp;
-            pen[rp * 32 + ((lane + rp / VS) & 31)] = Q[o];
-            pen[rv * 32 + ((lane + rv / VS) & 31)] = nx * Q[Np * 32 + o] + ny * Q[2 * Np * 32 + o] + nz * Q[3 * Np * 32 + o];
+            for (int r = 0; r < Nfp; ++r) qo[r] = qrow[r];
+          }
+#pragma unroll
+          for (int c = 0; c < REC / SW; ++c) {
+            VS_t x;
+            real* xs = reinterpret_cast<real*>(&x);
+#pragma unroll
+            for (int e = 0; e < SW; ++e) {
+              const int r = c * SW + e;                             // compile-time: p at position r, or n.v at position r - Nfp
+              const int o = QREG ? qo[QREG ? (r < Nfp ? r : r - Nfp) : 0] : qrow[r < Nfp ? r : r - Nfp];
+              if (r < Nfp) xs[e] = Ql[o];
+              else xs[e] = nx * Ql[Np * 32 + o] + ny * Ql[2 * Np * 32 + o] + nz * Ql[3 * Np * 32 + o];
+            }
+            out[c] = x;
           }
         }
       }
@@ -717,30 +765,20 @@ k_pipe(const __grid_constant__ StepArgs a) {
       // single-stage q ring: the last pass has gathered from Q, so the next item's q may land during the write-out
       if (QS == 1 && pass == (need_half ? 1 : 0) && more) issue_q(i + 1, 0);
       {  // cooperative write-out: the block's 32 x 4 records are one contiguous run; consecutive lanes store
-         // consecutive 16-byte pieces (piece P = element-lane P / NV, rows VS (P % NV) ..)
-        constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = ROWS / VS;
+         // consecutive 16-byte pieces (piece P = unit P % UE of element-lane P / UE): one vector load, one vector store
+        constexpr int VS = 16 / (int)sizeof(real), ROWS = 4 * REC, NV = SM::UE;
         using V = typename VecT<real, VS>::T;
         V* dst = reinterpret_cast<V*>(static_cast<real*>(pass == 0 ? L.qf_write[fi] : L.qf_half[fi]) + (size_t)b * 32 * ROWS);
         if constexpr (DUAL) {                   // register-bound: a rolled loop that recomputes the piece offsets
           for (int it = w; it < NV; it += NT) {
             const int P = it * 32 + lane, el = P / NV, o4 = P - el * NV;
-            V x;
-            real* xs = reinterpret_cast<real*>(&x);
-#pragma unroll
-            for (int e = 0; e < VS; ++e) xs[e] = pen[(o4 * VS + e) * 32 + ((el + o4) & 31)];
-            dst[P] = x;
+            dst[P] = *reinterpret_cast<const V*>(stg + (el * SM::SU + o4) * 16);
           }
         } else {
 #pragma unroll
           for (int k = 0; k < WOK; ++k) {
             const int it = w + k * NT;
-            if (it < NV) {
-              V x;
-              real* xs = reinterpret_cast<real*>(&x);
-#pragma unroll
-              for (int e = 0; e < VS; ++e) xs[e] = pen[wo_src[k] + e * 32];
-              dst[it * 32 + lane] = x;
-            }
+            if (it < NV) dst[it * 32 + lane] = *reinterpret_cast<const V*>(stg + wo_src[k]);
           }
         }
       }
