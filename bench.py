@@ -386,9 +386,14 @@ def extra_sweep(torch, device, peak, peak_src, hexes, traffic_table):
         sec, _ = timed_steps(g, torch, T, 3, 1, None, device)
         roof, ker, oth = profile_kernels(g, T, 1, dof // (4 * g.Np), g.Np, g.Nfp, prec // 8, peak, peak_src,
                                          traffic=lambda k, name=name, N=N, prec=prec: traffic_of(traffic_table, name, N, prec, k))
+        # in stream = CUDA events around the back-to-back launches of the timed region (the event pairs of `kernels` break
+        # the dependent-launch overlap); bytes = the algorithmic bytes of one global time step
+        nbytes = dof // (4 * g.Np) * algorithmic_scalars("step", g.Np, g.Nfp) * (prec // 8)
+        gbs = nbytes * 3 * T / sec * 1e-9
         out.append({"workload": name, "K": int(g.K), "N": N, "dtype": "f%d" % prec,
                     "levels": np.bincount(levels).tolist(), "value": dof * T * 3 / sec, "unit": UNIT,
-                    "ms_per_global_time_step": 1e3 * sec / (3 * T), "kernels": ker, **oth})
+                    "ms_per_global_time_step": 1e3 * sec / (3 * T), "achieved_gbs_in_stream": round(gbs, 1),
+                    "frac_in_stream": round(gbs / peak, 4), "kernels": ker, **oth})
         g.close()
         del g
         torch.cuda.empty_cache()
