@@ -400,7 +400,7 @@ def extra_sweep(torch, device, peak, peak_src, hexes, traffic_table):
     return out
 
 
-def extra_cfg5_sweep(torch, device, peak, hexes, nglobal=5):
+def extra_cfg5_sweep(torch, device, peak, hexes, nglobal=5, alu=None):
     """BASELINE.json config 5: 96 x 96 x 48 hexahedra x 6 tetrahedra, orders 1..6, fp32 and fp64, three multi-rate levels:
     DOF-updates/s and the fraction of the HBM roofline (algorithmic bytes of the fused step) per entry."""
     from workloads import make_config
@@ -420,6 +420,11 @@ def extra_cfg5_sweep(torch, device, peak, hexes, nglobal=5):
                         "single_rate_equivalent": 4 * int(g.K) * g.Np * (1 << (cfg["nlevels"] - 1)) * 2 * nglobal / sec,
                         "ms_per_global_time_step": 1e3 * sec / (2 * nglobal), "achieved_gbs": round(gbs, 1),
                         "frac": round(gbs / peak, 4), "workspace_gb": round(g.dg_workspace_bytes() * 1e-9, 2)})
+            if alu:     # the other roof: the method's flops (12 Np^2 + 32 Np Nfp per element evaluation) against the measured FMA ceiling
+                tf = dof // (4 * g.Np) * (12 * g.Np * g.Np + 32 * g.Np * g.Nfp) * 2 * nglobal / sec * 1e-12
+                pk_tf = max(alu["fp32_fma_tflops"], alu["fp32_ffma2_tflops"]) if prec == 32 else alu["fp64_fma_tflops"]
+                b = alu["fused_step_bound_by_order"]["N%d_f%d" % (N, prec)]["bound"]
+                out[-1].update({"bound": b, "achieved_tflops": round(tf, 2), "frac_alu": round(tf / pk_tf, 4)})
             g.close()
             del g
             torch.cuda.empty_cache()
@@ -728,7 +733,7 @@ def run_ours(args):
         line["sweep_large_mesh"] = extra_sweep(torch, device, peak, peak_src,
                                                {} if big else {"cfg4_rtm": (8, 8, 4), "cfg3_lts": (8, 8, 8)}, traffic_table)
         line["unfused_kernels"] = extra_unfused_kernels(torch, device, peak, None if big else (8, 8, 4), traffic_table)
-        line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8))
+        line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8), alu=line["peaks"])
         line["decomposition_one_gpu"] = extra_decomposition(torch, device, None if big else (8, 8, 4), 200 if big else 10)
         line["rtm_shot"] = extra_rtm_shot(torch, device, peak, peak_src, None if big else (8, 8, 4),
                                           None if big else 20, traffic_table)
