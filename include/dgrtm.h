@@ -160,6 +160,13 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n);
  * stream behind the step that wrote it, and the backward phase fetches the records it replays window - 1 evaluations
  * ahead.  Call before rtm_history_bytes / rtm_bind_history (it unbinds the RTM region).  Results are bit-identical to
  * the in-HBM history. */
+/* rtm_set_spill_packing(ctx, 1): the HOST copy of a spilled history keeps every value in half the bytes - fp64 -> fp32,
+ * fp32 -> bf16 (relative rounding 2^-24 / 2^-8 per value; the paper names compression of the boundary data as future work,
+ * PAPER.md:512).  Lossy: the reconstructed source wavefield and the image change at that level (documented with the
+ * measured error in DESIGN.md); the device ring and every kernel of the step keep full precision, the conversion runs on
+ * the copy stream; the replay takes EVERY record from the rounded copy (also those still in the ring), so one history
+ * gives one result.  Call before rtm_spill_bytes / rtm_set_trace_spill / rtm_history_bytes (it unbinds the RTM region). */
+int rtm_set_spill_packing(dg_ctx* ctx, int on);
 int rtm_spill_bytes(dg_ctx* ctx, int nsteps, size_t* n);
 int rtm_set_trace_spill(dg_ctx* ctx, void* host, size_t n, int window);
 /* Forward phase: from rest at t = 0, source on, nsteps global steps; captures the boundary traces,

@@ -60,6 +60,7 @@ SIGNATURES = {
     "dg_set_halo": (_i, [_vp, _i, _i64, _pi32, _pi64, _pi32]),
     "dg_halo_pull": (_i, [_vp, _i, _vp]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
+    "rtm_set_spill_packing": (_i, [_vp, _i]),
     "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
     "rtm_set_trace_spill": (_i, [_vp, _vp, _sz, _i]),
     "rtm_history_bytes": (_i, [_vp, _i, _psz]),
@@ -252,6 +253,9 @@ class DG:
 
     def rtm_set_trace_spill(self, host_ptr, nbytes, window):
         self._ck(_lib.rtm_set_trace_spill(self._h, _vp(host_ptr), nbytes, int(window)))
+
+    def rtm_set_spill_packing(self, on):
+        self._ck(_lib.rtm_set_spill_packing(self._h, int(bool(on))))
 
     def spill_traces_torch(self, nsteps, window):
         """Pinned host tensor for the whole trace history; the RTM region bound afterwards keeps a ring of `window`."""

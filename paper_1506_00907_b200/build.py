@@ -19,7 +19,7 @@ LIB = os.path.join(HERE, "libdgrtm.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC = os.path.join(CUDA_HOME, "bin", "nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-CUDA_SOURCES = ["fma_bench.cu", "noalloc.cu"]
+CUDA_SOURCES = ["fma_bench.cu", "noalloc.cu", "trace_pack.cu"]
 HOST_SOURCES = ["refelem.cpp", "mesh_setup.cpp", "api_core.cpp", "api_bind.cpp", "api_step.cpp",
                 "api_rtm.cpp", "api_get.cpp"]
 

@@ -18,9 +18,11 @@ int64_t device_records(const dg_ctx* c, int l, int nsteps) {
   return c->spill_window > 0 ? std::min<int64_t>(all, (int64_t)c->spill_window << l) : all;
 }
 size_t record_bytes(const dg_ctx* c, int l) { return c->model.stored[l].size() * (size_t)c->REC * c->rs; }
+// bytes of one record in the host copy: as on the device, or every value in half the bytes (rtm_set_spill_packing)
+size_t host_record_bytes(const dg_ctx* c, int l) { return c->spill_packed ? record_bytes(c, l) / 2 : record_bytes(c, l); }
 size_t spill_host_bytes(const dg_ctx* c, int nsteps) {
   size_t n = 0;
-  for (int l = 0; l < c->model.nlevels; ++l) n += ((size_t)records_of_level(c, l, nsteps) * record_bytes(c, l) + 255) / 256 * 256;
+  for (int l = 0; l < c->model.nlevels; ++l) n += ((size_t)records_of_level(c, l, nsteps) * host_record_bytes(c, l) + 255) / 256 * 256;
   return n;
 }
 void spill_release(dg_ctx* c) {
@@ -38,7 +40,7 @@ void spill_setup(dg_ctx* c, int nsteps) {
   size_t off = 0;
   for (int l = 0; l < c->model.nlevels; ++l) {
     c->hrec[l] = c->spill_host + off;
-    off += ((size_t)records_of_level(c, l, nsteps) * record_bytes(c, l) + 255) / 256 * 256;
+    off += ((size_t)records_of_level(c, l, nsteps) * host_record_bytes(c, l) + 255) / 256 * 256;
     const int64_t W = device_records(c, l, nsteps);
     c->slot_rec[l].assign((size_t)W, -1);
     c->ev_step[l].resize((size_t)W); c->ev_copy[l].resize((size_t)W);
@@ -76,6 +78,12 @@ void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
   const int Np = c->Np;
   for (int l = 0; l < md.nlevels; ++l)
     c->rec[l] = cv.take((size_t)device_records(c, l, nsteps) * md.stored[l].size() * c->REC * rs);
+  c->pack_stage = nullptr;
+  if (c->spill_window > 0 && c->spill_packed) {   // staging of one packed record (the largest level's)
+    size_t mx = 0;
+    for (int l = 0; l < md.nlevels; ++l) mx = std::max(mx, record_bytes(c, l) / 2);
+    c->pack_stage = cv.take(std::max<size_t>(mx, 16));
+  }
   const size_t nr = (size_t)std::max<int64_t>(1, std::max(c->nr, c->nr_reserve));   // receiver capacity
   c->d_data = cv.take(nr * ((size_t)nsteps * c->nlocal + 1) * rs);
   c->d_rcv_slot = (int*)cv.take(nr * 4);
@@ -98,18 +106,18 @@ void carve_history(dg_ctx* c, Carver& cv, int nsteps) {
 }
 
 struct HistPtrs {   // everything carve_history writes, for save / restore around a size query
-  char* rec[kMaxLevels]; char* d_data; int* a; int* b; char* cc; char* d; int* e; int* f; int* g; Field R; char* image; char* qfinal; int* ptr; char* ptv;
+  char* rec[kMaxLevels]; char* d_data; int* a; int* b; char* cc; char* d; int* e; int* f; int* g; Field R; char* image; char* qfinal; int* ptr; char* ptv; char* stage;
   void save(const dg_ctx* c) {
     for (int l = 0; l < kMaxLevels; ++l) rec[l] = c->rec[l];
     d_data = c->d_data; a = c->d_rcv_slot; b = c->d_rcv_level; cc = c->d_rcv_row; d = c->d_rcv_w;
     e = c->d_grp_slot; f = c->d_grp_off; g = c->d_grp_rcv; R = c->R; image = c->image; qfinal = c->qfinal;
-    ptr = c->d_pt_rcv; ptv = c->d_pt_val;
+    ptr = c->d_pt_rcv; ptv = c->d_pt_val; stage = c->pack_stage;
   }
   void restore(dg_ctx* c) const {
     for (int l = 0; l < kMaxLevels; ++l) c->rec[l] = rec[l];
     c->d_data = d_data; c->d_rcv_slot = a; c->d_rcv_level = b; c->d_rcv_row = cc; c->d_rcv_w = d;
     c->d_grp_slot = e; c->d_grp_off = f; c->d_grp_rcv = g; c->R = R; c->image = image; c->qfinal = qfinal;
-    c->d_pt_rcv = ptr; c->d_pt_val = ptv;
+    c->d_pt_rcv = ptr; c->d_pt_val = ptv; c->pack_stage = stage;
   }
 };
 
@@ -165,7 +173,13 @@ void spill_after_capture(dg_ctx* c, int l, int64_t j) {
   const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size()), nb = record_bytes(c, l);
   cuda_check(cudaEventRecord(c->ev_step[l][slot], c->stream), "cudaEventRecord");
   cuda_check(cudaStreamWaitEvent(c->copy_stream, c->ev_step[l][slot], 0), "cudaStreamWaitEvent");
-  cuda_check(cudaMemcpyAsync(c->hrec[l] + (size_t)j * nb, c->rec[l] + slot * nb, nb, cudaMemcpyDeviceToHost, c->copy_stream), "trace record D2H");
+  if (c->spill_packed) {   // pack on the copy stream into the staging record (stream order keeps it free), copy half the bytes
+    launch_trace_pack(c->rec[l] + slot * nb, c->pack_stage, nb / c->rs, c->precision, c->copy_stream);
+    cuda_check(cudaMemcpyAsync(c->hrec[l] + (size_t)j * (nb / 2), c->pack_stage, nb / 2, cudaMemcpyDeviceToHost, c->copy_stream), "packed trace record D2H");
+    c->slot_rec[l][slot] = -1;   // the replay takes every record from the (rounded) host copy, also the last W: one result per history
+  } else {
+    cuda_check(cudaMemcpyAsync(c->hrec[l] + (size_t)j * nb, c->rec[l] + slot * nb, nb, cudaMemcpyDeviceToHost, c->copy_stream), "trace record D2H");
+  }
   cuda_check(cudaEventRecord(c->ev_copy[l][slot], c->copy_stream), "cudaEventRecord");
 }
 namespace {
@@ -174,7 +188,12 @@ void spill_fetch(dg_ctx* c, int l, int64_t j) {
   const size_t slot = (size_t)(j % (int64_t)c->slot_rec[l].size()), nb = record_bytes(c, l);
   if (c->slot_rec[l][slot] == j) return;
   cuda_check(cudaStreamWaitEvent(c->copy_stream, c->ev_step[l][slot], 0), "cudaStreamWaitEvent");   // its last reader is done
-  cuda_check(cudaMemcpyAsync(c->rec[l] + slot * nb, c->hrec[l] + (size_t)j * nb, nb, cudaMemcpyHostToDevice, c->copy_stream), "trace record H2D");
+  if (c->spill_packed) {
+    cuda_check(cudaMemcpyAsync(c->pack_stage, c->hrec[l] + (size_t)j * (nb / 2), nb / 2, cudaMemcpyHostToDevice, c->copy_stream), "packed trace record H2D");
+    launch_trace_unpack(c->pack_stage, c->rec[l] + slot * nb, nb / c->rs, c->precision, c->copy_stream);
+  } else {
+    cuda_check(cudaMemcpyAsync(c->rec[l] + slot * nb, c->hrec[l] + (size_t)j * nb, nb, cudaMemcpyHostToDevice, c->copy_stream), "trace record H2D");
+  }
   cuda_check(cudaEventRecord(c->ev_copy[l][slot], c->copy_stream), "cudaEventRecord");
   c->slot_rec[l][slot] = j;
 }
@@ -255,6 +274,16 @@ int rtm_set_trace_spill(dg_ctx* ctx, void* host, size_t n, int window) {
   if (ctx->copy_stream) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
   ctx->spill_host = (char*)host; ctx->spill_bytes = host ? n : 0; ctx->spill_window = host ? window : 0;
   ctx->hist_bound = false;                     // the record layout of the RTM region changed: bind it again
+  DG_CATCH(ctx)
+}
+
+int rtm_set_spill_packing(dg_ctx* ctx, int on) {
+  DG_TRY(ctx)
+  if (on != 0 && on != 1) throw ApiError(DG_ERR_ARG, "on must be 0 or 1");
+  if (ctx->bound) sync_stream(ctx);
+  if (ctx->copy_stream) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
+  ctx->spill_packed = on != 0;
+  ctx->hist_bound = false;                     // host layout and the staging of the RTM region changed: bind it again
   DG_CATCH(ctx)
 }
 
@@ -404,8 +433,16 @@ int rtm_get_traces(dg_ctx* ctx, int level, int64_t record, double* buf) {
   if (ctx->spill_window > 0) {                 // the host copy is the history
     sync_stream(ctx);
     cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
-    const char* src = ctx->hrec[level] + (size_t)record * nf * ctx->REC * ctx->rs;
-    for (size_t i = 0; i < tmp.size(); ++i) tmp[i] = ctx->precision == 64 ? ((const double*)src)[i] : (double)((const float*)src)[i];
+    if (ctx->spill_packed) {                   // fp32 / bf16 values of the packed host copy
+      const char* src = ctx->hrec[level] + (size_t)record * nf * ctx->REC * (ctx->rs / 2);
+      for (size_t i = 0; i < tmp.size(); ++i) {
+        if (ctx->precision == 64) tmp[i] = (double)((const float*)src)[i];
+        else { const uint32_t bits = (uint32_t)((const uint16_t*)src)[i] << 16; float f; std::memcpy(&f, &bits, 4); tmp[i] = (double)f; }
+      }
+    } else {
+      const char* src = ctx->hrec[level] + (size_t)record * nf * ctx->REC * ctx->rs;
+      for (size_t i = 0; i < tmp.size(); ++i) tmp[i] = ctx->precision == 64 ? ((const double*)src)[i] : (double)((const float*)src)[i];
+    }
   } else {
     download_real(ctx, tmp.data(), ctx->rec[level] + (size_t)record * nf * ctx->REC * ctx->rs, tmp.size());
   }

@@ -168,6 +168,8 @@ struct dg_ctx {
   char* spill_host = nullptr;
   size_t spill_bytes = 0;
   int spill_window = 0;                     // records of the coarsest level on the device; 0 = no spill
+  bool spill_packed = false;                // the host copy keeps every value in half the bytes (rtm_set_spill_packing)
+  char* pack_stage = nullptr;               // device staging of one packed record (carved from the RTM region)
   char* hrec[dgrtm::kMaxLevels];            // per level: the host copy [nrec][nfaces][2][Nfp]
   cudaStream_t copy_stream = nullptr;
   std::vector<int64_t> slot_rec[dgrtm::kMaxLevels];   // record held (or being loaded) by every ring slot, -1 = none
@@ -229,6 +231,9 @@ void spill_before_capture(dg_ctx* c, int l, int64_t j);
 void spill_after_capture(dg_ctx* c, int l, int64_t j);
 void spill_before_replay(dg_ctx* c, int l, int64_t j);
 void spill_after_replay(dg_ctx* c, int l, int64_t j);
+// trace_pack.cu: n values of the device precision <-> n values of half the size (fp64 <-> fp32, fp32 <-> bf16)
+void launch_trace_pack(const void* src, void* dst, size_t n, int precision, cudaStream_t s);
+void launch_trace_unpack(const void* src, void* dst, size_t n, int precision, cudaStream_t s);
 void restart_history(dg_ctx* c);            // after dg_set_integrator / dg_set_dt
 
 struct RunOpts {
