@@ -122,7 +122,7 @@ int dg_static_scratch_bytes(size_t* n);
  * right-hand side until replaced.  Entries of faces of another type are ignored. */
 int dg_set_exterior(dg_ctx* ctx, const double* ext);
 
-/* ---- domain decomposition, single-rate -----------------------
+/* ---- domain decomposition ---------------------------------------
  * A sub-domain is an ordinary ctx over its part of the mesh whose cut faces are DG_BC_PRESCRIBED faces.  Their exterior
  * state is the neighbouring sub-domain's exposed trace at the coinciding node, fetched on the DEVICE by dg_halo_pull
  * straight from the neighbour's trace buffer (its own ctx on this GPU, or a peer pointer over NVLink): no host staging.
@@ -134,16 +134,35 @@ int dg_set_exterior(dg_ctx* ctx, const double* ext);
  *   boundary faces).
  * dg_get_trace_device: device pointer / size of the buffer that holds the exposed traces at the current time (it
  *   alternates between two buffers from step to step: query it before every dg_halo_pull).
- * dg_set_halo: halo set `set` (0..7, one per neighbouring sub-domain, filled in ascending order) of nh faces:
+ * dg_set_halo: halo set `set` (0..31, one per neighbouring sub-domain and level of the elements behind the cut, filled
+ *   in ascending order) of nh faces:
  *   bnd_index[nh] (boundary-face-list index here), src_record[nh] (record in that neighbour's buffer), src_pos[nh][Nfp]
  *   (position in that record of the node coinciding with my face node i).  After bind.
  * dg_halo_pull: enqueue the fetch of one set on this ctx's stream (the caller orders it after the neighbour's last step).
- * A time step of the decomposed problem = every sub-domain pulls, then every sub-domain takes dg_step(1). */
+ * A time step of the decomposed single-rate problem = every sub-domain pulls, then every sub-domain takes dg_step(1).
+ *
+ * Multi-rate sub-domains (the paper partitions the multi-rate scheme, cell weights 2^(l-1)):
+ * dg_set_model_levels: dg_set_model with the levels and the finest step of the WHOLE mesh imposed instead of derived from
+ *   this part alone: level[K] (0 = coarsest; face neighbours at most one apart), dt_local = step of the finest level,
+ *   bnd_level[nbnd] = level of the element behind each boundary face in the neighbouring sub-domain (-1: none; NULL: none
+ *   anywhere) - an element whose neighbour across the cut is finer exposes half-step traces (eq (19)) like one whose finer
+ *   neighbour is inside.
+ * dg_step_fine: advance nfine FINE steps of the multi-rate cycle (Alg. 1; fine step m of a global step advances the
+ *   levels whose step starts there); dg_step needs the scheme at the start of a global step.
+ * dg_get_trace_levels: current[nlevels] = the buffer that holds, for the elements of level l, the exposed traces at the
+ *   time level l has reached; half = the buffer of the half-step traces of the elements in mid-step; nbytes of each.
+ * Fine step m of the decomposed problem = every sub-domain pulls every set - from current[l] of the neighbour if the
+ *   level l of the elements behind that set starts a step at m, else from its half-step buffer - then every sub-domain
+ *   takes dg_step_fine(1) (paper_1506_00907_b200/decomp.py). */
 int dg_set_exterior_impedance(dg_ctx* ctx, const double* Zext);
 int dg_get_slots(dg_ctx* ctx, int64_t* slot_of);
 int dg_get_trace_device(dg_ctx* ctx, void** dptr, size_t* nbytes);
 int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, const int64_t* src_record, const int32_t* src_pos);
 int dg_halo_pull(dg_ctx* ctx, int set, const void* src_trace_device);
+int dg_set_model_levels(dg_ctx* ctx, const double* rho, const double* c, int nlevels, double dt_local, const int32_t* level,
+                        const int32_t* bnd_level);
+int dg_step_fine(dg_ctx* ctx, int nfine);
+int dg_get_trace_levels(dg_ctx* ctx, void** current /* [nlevels] */, void** half, size_t* nbytes);
 
 /* ---- RTM (Fig. 1) ---------------------------------------------------
  * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side

@@ -59,6 +59,9 @@ SIGNATURES = {
     "dg_get_trace_device": (_i, [_vp, C.POINTER(_vp), C.POINTER(_sz)]),
     "dg_set_halo": (_i, [_vp, _i, _i64, _pi32, _pi64, _pi32]),
     "dg_halo_pull": (_i, [_vp, _i, _vp]),
+    "dg_set_model_levels": (_i, [_vp, _pd, _pd, _i, _d, _pi32, _pi32]),
+    "dg_step_fine": (_i, [_vp, _i]),
+    "dg_get_trace_levels": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_sz)]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
     "rtm_set_spill_packing": (_i, [_vp, _i]),
     "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
@@ -241,6 +244,25 @@ class DG:
 
     def dg_halo_pull(self, halo_set, src_trace_device):
         self._ck(_lib.dg_halo_pull(self._h, int(halo_set), _vp(src_trace_device)))
+
+    def dg_set_model_levels(self, rho, c, nlevels, dt_local, level, bnd_level=None):
+        rho, c = _f64(rho), _f64(c)
+        level = np.ascontiguousarray(level, dtype=np.int32)
+        bnd_level = None if bnd_level is None else np.ascontiguousarray(bnd_level, dtype=np.int32)
+        assert rho.shape == (self.K,) and c.shape == (self.K,) and level.shape == (self.K,)
+        assert bnd_level is None or bnd_level.shape == (self.nbnd,)
+        self._ck(_lib.dg_set_model_levels(self._h, _ptr(rho, _pd), _ptr(c, _pd), int(nlevels), float(dt_local),
+                                          _ptr(level, _pi32), _ptr(bnd_level, _pi32)))
+
+    def dg_step_fine(self, nfine):
+        self._ck(_lib.dg_step_fine(self._h, int(nfine)))
+
+    def dg_get_trace_levels(self):
+        """([device pointer of the current traces of level l], device pointer of the half-step traces, bytes of each)."""
+        L = int(self.dg_get_dt()[1]).bit_length()                     # nlocal = 2^(L-1) fine steps per global step
+        cur, half, n = (_vp * 8)(), _vp(), _sz()
+        self._ck(_lib.dg_get_trace_levels(self._h, cur, C.byref(half), C.byref(n)))
+        return [cur[l] for l in range(L)], half.value, n.value
 
     # ---- RTM
     def rtm_set_receiver_capacity(self, max_receivers):

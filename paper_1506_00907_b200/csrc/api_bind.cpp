@@ -200,7 +200,7 @@ int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream) {
   cuda_check(cudaMemsetAsync(ctx->ws, 0, need, ctx->stream), "cudaMemsetAsync workspace");
   upload_tables(ctx);
   ctx->F.reset_history();
-  ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false; for (int x = 0; x < 9; ++x) ctx->halo_off[x] = 0;
+  ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false; for (int x = 0; x <= kMaxHaloSets; ++x) ctx->halo_off[x] = 0;
   ctx->have_final = false; ctx->have_backward = false;
   sync_stream(ctx);
   DG_CATCH(ctx)
@@ -246,16 +246,25 @@ int dg_get_trace_device(dg_ctx* ctx, void** dptr, size_t* nbytes) {
   DG_CATCH(ctx)
 }
 
+int dg_get_trace_levels(dg_ctx* ctx, void** current, void** half, size_t* nbytes) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (!current || !half || !nbytes) throw ApiError(DG_ERR_ARG, "current / half / nbytes is NULL");
+  for (int l = 0; l < ctx->model.nlevels; ++l) current[l] = ctx->F.qfb[ctx->F.par[l]];
+  *half = ctx->F.qfh;
+  *nbytes = trace_bytes(ctx);
+  DG_CATCH(ctx)
+}
+
 int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, const int64_t* src_record, const int32_t* src_pos) {
   DG_TRY(ctx)
   require_bound(ctx);
   const int64_t nb = (int64_t)ctx->mesh.bnd_k.size();
   const int Nfp = ctx->Nfp;
-  if (set < 0 || set > 7) throw ApiError(DG_ERR_ARG, "halo set must be in 0..7");
+  if (set < 0 || set >= kMaxHaloSets) throw ApiError(DG_ERR_ARG, "halo set must be in 0..31");
   const int64_t h0 = ctx->halo_off[set];          // sets are filled in ascending order: set s starts where s - 1 ended
   if (nh < 0 || h0 + nh > nb) throw ApiError(DG_ERR_ARG, "more halo faces than boundary faces");
   if (nh && (!bnd_index || !src_record || !src_pos)) throw ApiError(DG_ERR_ARG, "NULL table");
-  if (ctx->model.nlevels != 1) throw ApiError(DG_ERR_UNSUPPORTED, "the halo exchange is single-rate");
   for (int64_t h = 0; h < nh; ++h) {
     const int32_t bi = bnd_index[h];
     if (bi < 0 || bi >= nb) throw ApiError(DG_ERR_ARG, "boundary-face index out of range");
@@ -277,14 +286,14 @@ int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, cons
     cuda_check(cudaMemsetAsync(ctx->ext, 0, std::max<size_t>(1, (size_t)nb) * Nfp * 2 * ctx->rs, ctx->stream), "memset ext");
     ctx->has_ext = true;
   }
-  for (int x = set + 1; x < 9; ++x) ctx->halo_off[x] = h0 + nh;
+  for (int x = set + 1; x <= kMaxHaloSets; ++x) ctx->halo_off[x] = h0 + nh;
   DG_CATCH(ctx)
 }
 
 int dg_halo_pull(dg_ctx* ctx, int set, const void* src_trace_device) {
   DG_TRY(ctx)
   require_bound(ctx);
-  if (set < 0 || set > 7) throw ApiError(DG_ERR_ARG, "halo set must be in 0..7");
+  if (set < 0 || set >= kMaxHaloSets) throw ApiError(DG_ERR_ARG, "halo set must be in 0..31");
   if (!src_trace_device) throw ApiError(DG_ERR_ARG, "source trace buffer is NULL");
   const int64_t h0 = ctx->halo_off[set], nh = ctx->halo_off[set + 1] - h0;
   if (nh > 0) {

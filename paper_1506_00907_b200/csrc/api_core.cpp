@@ -326,6 +326,33 @@ int dg_set_model(dg_ctx* ctx, const double* rho, const double* c, int nlevels, d
   DG_CATCH(ctx)
 }
 
+int dg_set_model_levels(dg_ctx* ctx, const double* rho, const double* c, int nlevels, double dt_local, const int32_t* level,
+                        const int32_t* bnd_level) {
+  DG_TRY(ctx)
+  if (!rho || !c || !level) throw ApiError(DG_ERR_ARG, "rho / c / level is NULL");
+  if (nlevels < 1 || nlevels > kMaxLevels) throw ApiError(DG_ERR_UNSUPPORTED, "nlevels must be in 1..8");
+  if (!(dt_local > 0)) throw ApiError(DG_ERR_ARG, "dt_local must be positive");
+  const Mesh& m = ctx->mesh;
+  for (int64_t k = 0; k < m.K; ++k) {
+    if (!(rho[k] > 0) || !(c[k] > 0)) throw ApiError(DG_ERR_ARG, "rho and c must be positive (element " + std::to_string(k) + ")");
+    if (level[k] < 0 || level[k] >= nlevels) throw ApiError(DG_ERR_ARG, "level out of range (element " + std::to_string(k) + ")");
+  }
+  for (int64_t k = 0; k < m.K; ++k)
+    for (int f = 0; f < 4; ++f) {     // eq (19) serves neighbours one level apart
+      const int64_t k2 = m.EToE[4 * k + f];
+      const int l2 = k2 >= 0 ? level[k2] : (bnd_level && m.bnd_index[4 * k + f] >= 0 ? bnd_level[m.bnd_index[4 * k + f]] : -1);
+      if (l2 >= nlevels) throw ApiError(DG_ERR_ARG, "bnd_level out of range");
+      if (l2 >= 0 && std::abs(l2 - level[k]) > 1) throw ApiError(DG_ERR_ARG, "face neighbours must be at most one level apart");
+    }
+  const ImposedLevels imp{dt_local, level, bnd_level};
+  build_model(ctx->re, ctx->mesh, rho, c, nlevels, 1.0, ctx->model, &imp);
+  ctx->dt_local = ctx->model.dt_local;
+  ctx->nlocal = 1 << (nlevels - 1);
+  ctx->has_model = true;
+  ctx->bound = false; ctx->hist_bound = false;
+  DG_CATCH(ctx)
+}
+
 int dg_set_integrator(dg_ctx* ctx, int integrator) {
   DG_TRY(ctx)
   if (integrator != DG_INTEGRATOR_AB3 && integrator != DG_INTEGRATOR_LSERK4) throw ApiError(DG_ERR_ARG, "unknown integrator");

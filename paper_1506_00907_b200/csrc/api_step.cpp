@@ -59,7 +59,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     p.nr = (int)c->nr; p.rcv_slot = c->d_rcv_slot; p.rcv_row = c->d_rcv_row; p.rcv_level = c->d_rcv_level;
     p.data = c->d_data; p.nsamp = nsamp; p.sample = jabs;
     for (int l = 0; l < L; ++l) {
-      const int off = (int)(m % stride[l]);
+      const int off = (int)((m + o.fine_phase) % stride[l]);
       if (!off) continue;
       const int order = o.fields[0]->nhist[l];
       double w[3] = {0, 0, 0};
@@ -92,7 +92,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   }
   for (int l = 0; l < L; ++l) a.lv[l].blk_end = md.lvl_blk0[l] + md.lvl_nblk[l];
 
-  const int64_t nfine = (int64_t)nglobal * nloc;
+  const int64_t nfine = o.nfine >= 0 ? o.nfine : (int64_t)nglobal * nloc;
   for (int64_t m = 0; m < nfine; ++m) {
     const int64_t jabs = o.first_fine + dir * m;
     const double t_start = o.t0 + dir * (double)m * dtl;
@@ -105,7 +105,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
       DG_LAUNCH(c, KC_INJECT, c->kt->inject(p, c->stream));
     }
     int lmin = L - 1;
-    while (lmin > 0 && m % stride[lmin - 1] == 0) --lmin;   // strides are powers of two
+    while (lmin > 0 && (m + o.fine_phase) % stride[lmin - 1] == 0) --lmin;   // strides are powers of two
     for (int l = 0; l < L; ++l) {
       StepLevel& S = a.lv[l];
       const bool active = l >= lmin;
@@ -216,12 +216,28 @@ int dg_step(dg_ctx* ctx, int nsteps) {
     run_lserk4(ctx, nsteps);
     ctx->fine += nsteps;
   } else {
+    if (ctx->fine % ctx->nlocal) throw ApiError(DG_ERR_STATE, "dg_step_fine left the scheme inside a global step: finish it first");
     RunOpts o;
     o.direction = 1; o.fields[0] = &ctx->F; o.nfields = 1; o.source_on[0] = ctx->has_src;
     o.first_fine = ctx->fine; o.t0 = ctx->t0 + (double)ctx->fine * ctx->dt_local;
     run_mrab(ctx, nsteps, o);
     ctx->fine += (int64_t)nsteps * ctx->nlocal;
   }
+  check_launches(ctx);
+  DG_CATCH(ctx)
+}
+
+int dg_step_fine(dg_ctx* ctx, int nfine) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (nfine < 0) throw ApiError(DG_ERR_ARG, "nfine must be >= 0");
+  if (ctx->integrator != DG_INTEGRATOR_AB3) throw ApiError(DG_ERR_STATE, "dg_step_fine advances the multi-rate AB scheme");
+  RunOpts o;
+  o.direction = 1; o.fields[0] = &ctx->F; o.nfields = 1; o.source_on[0] = ctx->has_src;
+  o.first_fine = ctx->fine; o.t0 = ctx->t0 + (double)ctx->fine * ctx->dt_local;
+  o.fine_phase = ctx->fine % ctx->nlocal; o.nfine = nfine;
+  run_mrab(ctx, 0, o);
+  ctx->fine += nfine;
   check_launches(ctx);
   DG_CATCH(ctx)
 }

@@ -18,6 +18,7 @@
 namespace dgrtm {
 
 constexpr int kMaxLevels = 8;
+constexpr int kMaxHaloSets = 32;   // (neighbouring sub-domain, level of the elements behind the cut) pairs of one sub-domain
 
 // kernel classes of the launch counter / per-kernel timing (dg_get_kernel_times)
 enum KernelClass { KC_RHS = 0, KC_UPDATE, KC_HALO, KC_IMAGE, KC_SOURCE, KC_RECORD, KC_INJECT, KC_CAPTURE, KC_RK, KC_STEP, KC_STEP_IMAGE, KC_COUNT };
@@ -136,7 +137,7 @@ struct dg_ctx {
   int* d_pt_src = nullptr;                  // per slot: 0 at the source element, else -1
   // ---- halo faces of a domain decomposition (dg_set_halo): tables [bnd | rec | pos] in one carved region
   char* d_halo = nullptr;
-  int64_t halo_off[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // faces of halo set s (one set per neighbouring sub-domain): [halo_off[s], halo_off[s+1])
+  int64_t halo_off[dgrtm::kMaxHaloSets + 1] = {};   // faces of halo set s (one set per neighbouring sub-domain): [halo_off[s], halo_off[s+1])
   std::vector<double> bnd_Zext;             // exterior impedance per boundary face (> 0: Z_f = (Z- + Zext) / 2), dg_set_exterior_impedance
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
@@ -243,6 +244,7 @@ struct RunOpts {
   bool source_on[2] = {false, false};
   bool capture = false, replay = false, record = false;
   int inject_field = -1;
+  int64_t fine_phase = 0, nfine = -1;        // dg_step_fine: fine index within the cycle at the start, fine steps to run (-1: whole global steps)
   bool image = false;
   int imaging = DG_IMAGING_CHARACTERISTIC;
   double updir[3] = {0, 0, -1};

@@ -164,7 +164,7 @@ std::string build_mesh(const RefElem& re, int64_t K, int64_t Nv, const int32_t* 
 }
 
 void build_model(const RefElem& re, const Mesh& m, const double* rho, const double* c, int nlevels, double cfl,
-                 Model& md) {
+                 Model& md, const ImposedLevels* imp) {
   const int64_t K = m.K;
   const int N = re.N, L = nlevels;
   md.rho.assign(rho, rho + K); md.c.assign(c, c + K);
@@ -196,6 +196,16 @@ void build_model(const RefElem& re, const Mesh& m, const double* rho, const doub
     }
   md.level.resize(K);
   for (int64_t k = 0; k < K; ++k) md.level[k] = (L - 1) - j[k];
+  if (imp) {   // a sub-domain of a decomposition: the levels and the step of the WHOLE mesh (dg_set_model_levels)
+    md.dt_local = imp->dt_local;
+    for (int64_t k = 0; k < K; ++k) md.level[k] = imp->level[k];
+  }
+  // level of the element behind a boundary face in the neighbouring sub-domain (-1: none)
+  auto outer_level = [&](int64_t k, int f) -> int {
+    if (!imp || !imp->bnd_level) return -1;
+    const int32_t b = m.bnd_index[4 * k + f];
+    return b < 0 ? -1 : imp->bnd_level[b];
+  };
 
   // ---- slot layout
   md.lvl_blk0.assign(L, 0); md.lvl_nblk.assign(L, 0); md.lvl_count.assign(L, 0);
@@ -216,6 +226,7 @@ void build_model(const RefElem& re, const Mesh& m, const double* rho, const doub
     for (int f = 0; f < 4; ++f) {
       const int64_t k2 = m.EToE[4 * k + f];
       if (k2 >= 0 && md.level[k2] > md.level[k]) return true;
+      if (k2 < 0 && outer_level(k, f) > md.level[k]) return true;
     }
     return false;
   };
@@ -235,6 +246,7 @@ void build_model(const RefElem& re, const Mesh& m, const double* rho, const doub
       for (int f = 0; f < 4; ++f) {
         const int64_t k2 = m.EToE[4 * k + f];
         if (k2 >= 0 && md.level[k2] > md.level[k]) finer = true;
+        if (k2 < 0 && outer_level(k, f) > md.level[k]) finer = true;
       }
       if (finer) md.coarse_nb[l].push_back((int32_t)s);
     }

@@ -43,8 +43,11 @@ struct Model {
   std::vector<std::vector<int32_t>> stored;      // per level: boundary-list indices of absorbing faces
 };
 
+// levels and local step imposed from outside (a sub-domain takes those of the whole mesh, dg_set_model_levels);
+// bnd_level[nbnd]: level of the element behind a boundary face in the neighbouring sub-domain, -1 = none (may be NULL)
+struct ImposedLevels { double dt_local; const int32_t* level; const int32_t* bnd_level; };
 void build_model(const RefElem& re, const Mesh& m, const double* rho, const double* c, int nlevels, double cfl,
-                 Model& md);
+                 Model& md, const ImposedLevels* imp = nullptr);
 
 // element containing x (lowest id with all barycentrics >= -1e-10, reading Q11) and its (r,s,t); -1 if none.
 // Candidates come from a uniform grid over the element bounding boxes, built on first use.

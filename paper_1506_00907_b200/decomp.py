@@ -1,7 +1,7 @@
-"""Domain decomposition of the single-rate scheme over several sub-domains:
+"""Domain decomposition of the (single- or multi-rate) scheme over several sub-domains:
 set-up only - partition, local meshes, halo tables.  Every step of the path still runs in the library's kernels: a
 sub-domain is an ordinary `DG` context whose cut faces are prescribed-exterior faces, and their exterior states are
-fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_halo) before every step.
+fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_halo) before every (fine) step.
 
     part = partition_elements(EToV, VX, nparts, weights)         # weighted recursive coordinate bisection
     dd = Decomposition(N, precision, EToV, VX, rho, c, part)     # one DG context per part, halo tables
@@ -9,7 +9,9 @@ fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_hal
 
 The paper partitions with METIS, cell weights 2^(l-1) and keeps the finest cells off the cuts
 (PAPER.md:387); METIS is not in this container: `partition_elements` is a weighted coordinate bisection that takes the same
-weights.  `Decomposition` keeps all sub-domains in one process (on one GPU their launches are ordered by the shared stream).
+weights and the same lumping of the finest cells with their neighbours.  With nlevels > 1 a sub-domain takes the levels of
+the whole mesh (dg_set_model_levels), the exchange runs before every FINE step (dg_step_fine) and reads, per halo set, the
+neighbour's current traces of that set's level or - the level being in mid-step - its half-step traces (eq (19)).  `Decomposition` keeps all sub-domains in one process (on one GPU their launches are ordered by the shared stream).
 `RankDecomposition` is the one-process-per-sub-domain mode (one rank of torch.distributed = one sub-domain = one GPU): the
 ranks exchange CUDA IPC handles of their workspaces once, after which the source pointer of `dg_halo_pull` is the peer
 mapping of the neighbour's trace buffer - the loads of k_halo cross NVLink (or stay on the device when the ranks share a
@@ -23,12 +25,59 @@ from .binding import DG
 BC_PRESCRIBED = 4
 
 
-def partition_elements(EToV, VX, nparts, weights=None):
+def face_neighbours(EToV):
+    """[K][4] element behind each face (-1: boundary), faces matched by their sorted vertex triples (the order of the four
+    faces of an element is the order of the vertex left out and plays no role for the partition)."""
+    EToV = np.asarray(EToV)
+    K = EToV.shape[0]
+    tri = np.sort(np.stack([np.delete(EToV, v, axis=1) for v in range(4)], axis=1).reshape(4 * K, 3), axis=1)
+    order = np.lexsort((tri[:, 2], tri[:, 1], tri[:, 0]))
+    same = np.all(tri[order[1:]] == tri[order[:-1]], axis=1)
+    nb = np.full(4 * K, -1, dtype=np.int64)
+    a, b = order[:-1][same], order[1:][same]
+    nb[a], nb[b] = b // 4, a // 4
+    return nb.reshape(K, 4)
+
+
+def lump_groups(lump, nb):
+    """Group id per element (-1: none): every element flagged in `lump` together with its face neighbours; groups that
+    share an element are merged ("lumping each finest element (or group of finest elements) with his
+    neighbors")."""
+    K = nb.shape[0]
+    root = np.arange(K)
+
+    def find(x):
+        while root[x] != x:
+            root[x] = root[root[x]]
+            x = root[x]
+        return x
+
+    member = np.zeros(K, dtype=bool)
+    for k in np.nonzero(lump)[0]:
+        member[k] = True
+        for k2 in nb[k]:
+            if k2 >= 0:
+                member[k2] = True
+                ra, rb = find(k), find(int(k2))
+                if ra != rb:
+                    root[max(ra, rb)] = min(ra, rb)
+    return np.array([find(k) if member[k] else -1 for k in range(K)], dtype=np.int64)
+
+
+def partition_elements(EToV, VX, nparts, weights=None, lump=None):
     """Part id per element by recursive coordinate bisection of the element centroids along the longest axis, each cut
-    balancing the summed weights (weight = local steps per global step of the cell)."""
+    balancing the summed weights (weight = local steps per global step of the cell).  lump: boolean mask of
+    elements (the finest level's) that must not touch a cut: each is lumped with its face neighbours into one point
+    before the bisection and separated afterwards, so that the fine steps that advance the finest level
+    alone need no exchange."""
     K = EToV.shape[0]
     cen = VX[EToV].mean(axis=1)
     w = np.ones(K) if weights is None else np.asarray(weights, dtype=np.float64)
+    if lump is not None and np.any(lump):
+        grp = lump_groups(np.asarray(lump, dtype=bool), face_neighbours(EToV))
+        for gid in np.unique(grp[grp >= 0]):
+            m = grp == gid
+            cen[m] = (cen[m] * w[m, None]).sum(axis=0) / w[m].sum()   # one point: a cut cannot separate its members
     part = np.zeros(K, dtype=np.int32)
 
     def split(idx, p0, n):
@@ -36,11 +85,24 @@ def partition_elements(EToV, VX, nparts, weights=None):
             part[idx] = p0
             return
         ext = cen[idx].max(axis=0) - cen[idx].min(axis=0)
-        order = idx[np.argsort(cen[idx, int(np.argmax(ext))], kind="stable")]
+        axis = int(np.argmax(ext))
+        order = idx[np.lexsort((cen[idx, (axis + 2) % 3], cen[idx, (axis + 1) % 3], cen[idx, axis]))]
         nl = n // 2
         cw = np.cumsum(w[order])
         cut = int(np.searchsorted(cw, cw[-1] * nl / n)) + 1
         cut = min(max(cut, 1), len(order) - 1)
+        same = np.all(cen[order[1:]] == cen[order[:-1]], axis=1)      # members of one lump are adjacent in `order`
+        if same[cut - 1]:                                             # the cut falls inside a lump: move it to the nearer end
+            lo, hi = cut, cut
+            while lo > 1 and same[lo - 1]:
+                lo -= 1
+            lo = lo if not same[lo - 1] else 0
+            while hi < len(order) - 1 and same[hi - 1]:
+                hi += 1
+            hi = hi if not same[hi - 1] else len(order)
+            cands = [c for c in (lo, hi) if 1 <= c <= len(order) - 1]
+            if cands:
+                cut = min(cands, key=lambda c: abs(c - cut))
         split(order[:cut], p0, nl)
         split(order[cut:], p0 + nl, n - nl)
 
@@ -51,18 +113,21 @@ def partition_elements(EToV, VX, nparts, weights=None):
 class Decomposition:
     """The sub-domains of one mesh as DG contexts with their halo tables.  Global arrays in, global arrays out."""
 
-    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15, only=None):
-        """only = p: bind / step sub-domain p alone (the others exist on the host for their slot tables)."""
+    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15, only=None, nlevels=1):
+        """only = p: bind / step sub-domain p alone (the others exist on the host for their slot tables).
+        nlevels > 1: the multi-rate scheme; the levels and the finest step are those of the WHOLE mesh."""
         self.only = only
+        self.nlevels, self.nlocal = int(nlevels), 1 << (int(nlevels) - 1)
         EToV = np.ascontiguousarray(EToV, dtype=np.int32)
         self.K, self.part = EToV.shape[0], np.asarray(part, dtype=np.int32)
         self.nparts = int(self.part.max()) + 1
         assert self.nparts <= 9, "a sub-domain has at most 8 halo sets"
         # global connectivity and the global stable step from a host-only context of the whole mesh
         g = DG(N, precision, EToV, VX, face_bc=face_bc, default_bc=default_bc)
-        g.dg_set_model(rho, c, 1, cfl)
+        g.dg_set_model(rho, c, self.nlevels, cfl)
         EToE, EToF, mapP = g.dg_get_connectivity()
         self.dt = g.dg_get_dt()[0]
+        self.level = g.dg_get_levels()
         self.Np, self.Nfp = g.Np, g.Nfp
         g.close()
         self.elems = [np.nonzero(self.part == p)[0] for p in range(self.nparts)]
@@ -80,10 +145,11 @@ class Decomposition:
             fbc = np.full((e.size, 4), default_bc, dtype=np.int8) if face_bc is None else np.array(face_bc[e], dtype=np.int8)
             fbc[cut] = BC_PRESCRIBED
             s = DG(N, precision, etov, VX[verts], face_bc=fbc, default_bc=default_bc)
-            s.dg_set_model(np.asarray(rho)[e], np.asarray(c)[e], 1, cfl)
             bk, bf, bc = s.dg_get_boundary_faces()
             k2 = nb[bk, bf]                                           # global neighbour behind every boundary face
             halo = (k2 >= 0) & (bc == BC_PRESCRIBED)
+            s.dg_set_model_levels(np.asarray(rho)[e], np.asarray(c)[e], self.nlevels, self.dt, self.level[e],
+                                  np.where(halo, self.level[np.maximum(k2, 0)], -1))
             s.dg_set_exterior_impedance(np.where(halo, Z[np.maximum(k2, 0)], 0.0))
             self.sub.append(s)
             self._halo.append((bk, bf, k2, halo))
@@ -92,21 +158,30 @@ class Decomposition:
 
     def _tables(self, EToF, mapP):
         slots = [s.dg_get_slots() for s in self.sub]
-        self.sets = []                                               # per sub-domain: list of (neighbour part, tables)
+        self.sets = []                                               # per sub-domain: list of (neighbour part, tables),
+        self.set_level = []                                          # one set per neighbour and level of the elements behind
+        self.set_mine = []
+        self.pulls = np.zeros(self.nlocal, dtype=np.int64)           # halo fetches enqueued per fine step of the cycle
         for p, s in enumerate(self.sub):
             bk, bf, k2, halo = self._halo[p]
             ge = self.elems[p][bk]                                    # global element of every boundary face
-            sets = []
+            sets, levels, mine = [], [], []
             for q in range(self.nparts):
-                sel = np.nonzero(halo & (self.part[np.maximum(k2, 0)] == q))[0]
-                if q == p or sel.size == 0:
-                    continue
-                f2 = EToF[ge[sel], bf[sel]]
-                rec = slots[q][self.local[k2[sel]]] * 4 + f2
-                pos = mapP[ge[sel], bf[sel]]                          # [nh][Nfp]: neighbour's face node at my node i
-                sets.append((q, sel.astype(np.int32), rec.astype(np.int64), pos.astype(np.int32)))
-            assert len(sets) <= 8
+                for lev in range(self.nlevels):
+                    k2c = np.maximum(k2, 0)
+                    sel = np.nonzero(halo & (self.part[k2c] == q) & (self.level[k2c] == lev))[0]
+                    if q == p or sel.size == 0:
+                        continue
+                    f2 = EToF[ge[sel], bf[sel]]
+                    rec = slots[q][self.local[k2[sel]]] * 4 + f2
+                    pos = mapP[ge[sel], bf[sel]]                      # [nh][Nfp]: neighbour's face node at my node i
+                    sets.append((q, sel.astype(np.int32), rec.astype(np.int64), pos.astype(np.int32)))
+                    levels.append(lev)
+                    mine.append(int(self.level[ge[sel]].max()))       # finest of MY elements on these faces
+            assert len(sets) <= 32
             self.sets.append(sets)
+            self.set_level.append(levels)
+            self.set_mine.append(mine)
 
     # ---- memory, set-up
     def mine(self):
@@ -116,7 +191,6 @@ class Decomposition:
         for p in self.mine():
             s = self.sub[p]
             s.bind_torch(device)
-            s.dg_set_dt(self.dt)                                      # the global stable step, not the sub-domain's own
             for i, (q, bnd, rec, pos) in enumerate(self.sets[p]):
                 s.dg_set_halo(i, bnd, rec, pos)
         self._bound = True
@@ -141,15 +215,28 @@ class Decomposition:
             q[self.elems[p]] = s.dg_get_fields()
         return q
 
-    # ---- the step: every sub-domain pulls its halo, then every sub-domain advances
+    # ---- the step: every sub-domain pulls its halo, then every sub-domain advances one FINE step (Alg. 1)
+    def first_level_starting_at(self, m):
+        """Coarsest level whose step starts at fine step m of a global step (level l takes 2^(L-1-l) fine steps)."""
+        lmin = self.nlevels - 1
+        while lmin > 0 and m % (1 << (self.nlevels - lmin)) == 0:
+            lmin -= 1
+        return lmin
+
     def dg_step(self, nsteps):
         for _ in range(int(nsteps)):
-            src = [s.dg_get_trace_device()[0] for s in self.sub]
-            for p, s in enumerate(self.sub):
-                for i, (q, _, _, _) in enumerate(self.sets[p]):
-                    s.dg_halo_pull(i, src[q])
-            for s in self.sub:
-                s.dg_step(1)
+            for m in range(self.nlocal):
+                lmin = self.first_level_starting_at(m)
+                tr = [s.dg_get_trace_levels() for s in self.sub]
+                for p, s in enumerate(self.sub):
+                    for i, (q, _, _, _) in enumerate(self.sets[p]):
+                        if self.set_mine[p][i] < lmin:          # none of my elements on these faces steps now (with the
+                            continue                            # finest level off the cuts: no exchange at odd fine steps)
+                        lev = self.set_level[p][i]              # traces at the time the fine levels have reached: the
+                        s.dg_halo_pull(i, tr[q][0][lev] if lev >= lmin else tr[q][1])   # level's own, or its half-step ones
+                        self.pulls[m] += 1
+                for s in self.sub:
+                    s.dg_step_fine(1)
 
     def launch_count(self):
         return sum(s.dg_get_launch_count() for s in self.sub)
@@ -184,24 +271,32 @@ class RankDecomposition(Decomposition):
         self.dist.barrier()
 
     def _trace_offsets(self):
-        """Offset of every rank's current trace buffer inside its workspace tensor (a host-side all-gather)."""
+        """Offsets of every rank's trace buffers (current one per level, half-step one) inside its workspace tensor
+        (a host-side all-gather)."""
         me = self.sub[self.rank]
-        off = me.dg_get_trace_device()[0] - me._ws.data_ptr()
+        cur, half, _ = me.dg_get_trace_levels()
+        base = me._ws.data_ptr()
         offs = [None] * self.nparts
-        self.dist.all_gather_object(offs, int(off))
+        self.dist.all_gather_object(offs, ([int(c - base) for c in cur], int(half - base)))
         return offs
 
     def dg_step(self, nsteps):
         import torch
         me = self.sub[self.rank]
         for _ in range(int(nsteps)):
-            offs = self._trace_offsets()            # also orders this step after every rank's previous step (see below)
-            for i, (q, _, _, _) in enumerate(self.sets[self.rank]):
-                me.dg_halo_pull(i, self._peer[q].data_ptr() + offs[q])
-            torch.cuda.synchronize(self._device)    # my fetches have read the neighbours' traces ...
-            self.dist.barrier()                     # ... on every rank, before anybody's step overwrites them
-            me.dg_step(1)
-            torch.cuda.synchronize(self._device)    # my new traces are complete before the next all-gather returns
+            for m in range(self.nlocal):
+                lmin = self.first_level_starting_at(m)
+                offs = self._trace_offsets()        # also orders this step after every rank's previous step (see below)
+                for i, (q, _, _, _) in enumerate(self.sets[self.rank]):
+                    if self.set_mine[self.rank][i] < lmin:
+                        continue
+                    lev = self.set_level[self.rank][i]
+                    self.pulls[m] += 1
+                    me.dg_halo_pull(i, self._peer[q].data_ptr() + (offs[q][0][lev] if lev >= lmin else offs[q][1]))
+                torch.cuda.synchronize(self._device)    # my fetches have read the neighbours' traces ...
+                self.dist.barrier()                     # ... on every rank, before anybody's step overwrites them
+                me.dg_step_fine(1)
+                torch.cuda.synchronize(self._device)    # my new traces are complete before the next all-gather returns
 
     def dg_set_state(self, q, t0=0.0):
         self.sub[self.rank].dg_set_state(q[self.elems[self.rank]], t0)

@@ -6,7 +6,7 @@ import sys
 import numpy as np
 
 
-def run(rank, world, port, N, precision, nsteps, hexes, out_path):
+def run(rank, world, port, N, precision, nsteps, hexes, out_path, workload="cfg2_two_layer"):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     import torch
@@ -16,11 +16,11 @@ def run(rank, world, port, N, precision, nsteps, hexes, out_path):
     sys.path.insert(0, os.path.dirname(here))
     from workloads import make_config
     from paper_1506_00907_b200.decomp import RankDecomposition, partition_elements
-    cfg = make_config("cfg2_two_layer", hexes=hexes, N=N, nsteps=nsteps)
+    cfg = make_config(workload, hexes=hexes, N=N, nsteps=nsteps)
     cfg["source"] = dict(cfg["source"], f0=40.0, tp=0.01)
     part = partition_elements(cfg["EToV"], cfg["VX"], world)
     dd = RankDecomposition(dist, N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
-                           default_bc=cfg["default_bc"])
+                           default_bc=cfg["default_bc"], nlevels=cfg["nlevels"], cfl=cfg["cfl"])
     torch.cuda.set_device(0)
     dd.bind_torch("cuda:0")
     s = cfg["source"]

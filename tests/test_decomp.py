@@ -102,6 +102,109 @@ def test_decomposed_run_matches_the_oracle(N, precision, nparts):
     assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
 
 
+def _lts_cfg(N, hexes=(6, 6, 8), nsteps=100):
+    cfg = make_config("cfg3_lts", hexes=hexes, N=N, nsteps=nsteps)
+    cfg["source"] = dict(cfg["source"], f0=40.0, tp=0.01)
+    return cfg
+
+
+def test_multirate_halo_sets_carry_one_level_each():
+    """Host logic of the multi-rate decomposition: the sub-domains take the levels of the whole mesh (also where a part
+    alone would grade differently), weights 2^l balance the local steps, every halo set points at elements
+    of ONE level of the neighbour, and an element whose finer neighbour lies across the cut is laid out among the
+    elements that expose half-step traces (first slots of its level)."""
+    from paper_1506_00907_b200.decomp import Decomposition, partition_elements
+    import paper_1506_00907_b200 as pk
+    cfg = _lts_cfg(2)
+    g = pk.DG(cfg["N"], 64, cfg["EToV"], cfg["VX"], default_bc=cfg["default_bc"])
+    g.dg_set_model(cfg["rho"], cfg["c"], cfg["nlevels"], cfg["cfl"])
+    level, EToE = g.dg_get_levels(), g.dg_get_connectivity()[0]
+    g.close()
+    assert len(np.unique(level)) == 3
+    part = partition_elements(cfg["EToV"], cfg["VX"], 3, 2.0 ** level)
+    work = np.array([(2.0 ** level[part == p]).sum() for p in range(3)])
+    assert work.max() / work.mean() < 1.1, work
+    dd = Decomposition(cfg["N"], 64, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"],
+                       nlevels=3, cfl=cfg["cfl"])
+    cross = 0
+    for p, s in enumerate(dd.sub):
+        assert np.array_equal(s.dg_get_levels(), level[dd.elems[p]])
+        assert s.dg_get_dt() == (dd.dt, 4)                             # the finest step of the whole mesh, 2^(L-1) per global step
+        slots = [x.dg_get_slots() for x in dd.sub]
+        bk, bf, bc = s.dg_get_boundary_faces()
+        for i, (q, bnd, rec, pos) in enumerate(dd.sets[p]):
+            lev = dd.set_level[p][i]
+            behind = {int(sl): k for k, sl in enumerate(slots[q])}
+            for h in range(bnd.size):
+                assert level[dd.elems[q][behind[int(rec[h] // 4)]]] == lev
+                mine = level[dd.elems[p][bk[bnd[h]]]]
+                assert abs(int(mine) - lev) <= 1
+                cross += mine != lev
+        # elements with a finer neighbour, inside or across the cut, come first within their level
+        sl = s.dg_get_slots()
+        for lev in range(3):
+            e = dd.elems[p][level[dd.elems[p]] == lev]
+            if e.size == 0:
+                continue
+            nbl = np.where(EToE[e] >= 0, level[np.maximum(EToE[e], 0)], -1)
+            finer = (nbl > lev).any(axis=1)
+            order = np.argsort(sl[dd.local[e]])
+            assert not np.any(np.diff(finer[order].astype(int)) > 0)       # all True, then all False
+    assert cross > 0                                                   # the cuts do cross level interfaces
+    dd.close()
+    # finest-level elements lumped with their neighbours before the bisection (PAPER.md:387): none of their faces is cut,
+    # the weights stay balanced
+    from paper_1506_00907_b200.decomp import face_neighbours
+    assert np.array_equal(np.sort(face_neighbours(cfg["EToV"]), axis=1), np.sort(EToE, axis=1))
+    cut_faces = lambda part: sum(1 for k in np.nonzero(level == 2)[0] for k2 in EToE[k] if k2 >= 0 and part[k2] != part[k])
+    plain = partition_elements(cfg["EToV"], cfg["VX"], 5, 2.0 ** level)
+    lumped = partition_elements(cfg["EToV"], cfg["VX"], 5, 2.0 ** level, lump=level == 2)
+    assert cut_faces(plain) > 0 and cut_faces(lumped) == 0
+    work = np.array([(2.0 ** level[lumped == p]).sum() for p in range(5)])
+    assert work.max() / work.mean() < 1.1, work
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("N,precision,nparts,lump", [(3, 64, 2, False), (2, 64, 5, False), (2, 64, 5, True), (3, 32, 3, True),
+                                                     (4, 32, 2, False)])
+def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump):
+    """Three levels, cuts across level interfaces: before every FINE step each sub-domain fetches, per halo set, the
+    neighbour's traces of that set's level - its current ones if the level starts a step there, its half-step ones (eq (19))
+    if it is in mid-step - and advances by dg_step_fine(1).  Same fields as the single-domain oracle and library runs."""
+    from paper_1506_00907_b200.decomp import Decomposition, partition_elements
+    cfg = _lts_cfg(N)
+    nsteps = cfg["nsteps"]
+    o = make_oracle(cfg)
+    part = partition_elements(cfg["EToV"], cfg["VX"], nparts, 2.0 ** np.asarray(o.level),
+                              lump=(np.asarray(o.level) == 2) if lump else None)
+    dd = Decomposition(N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"],
+                       nlevels=cfg["nlevels"], cfl=cfg["cfl"])
+    assert np.array_equal(dd.level, o.level)
+    assert any(dd.set_level[p][i] != lev for p in range(nparts) for i, (q, bnd, _, _) in enumerate(dd.sets[p])
+               for lev in dd.level[dd.elems[p][dd.sub[p].dg_get_boundary_faces()[0][bnd]]])
+    dd.bind_torch("cuda:0")
+    s = cfg["source"]
+    dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+    dd.dg_step(nsteps)
+    q = dd.dg_get_fields()
+    assert dd.pulls[0] > 0 and dd.pulls[2] > 0
+    if lump:                                                           # the finest level is off the cuts: the fine steps that
+        assert dd.pulls[1] == 0 and dd.pulls[3] == 0                   # advance it alone exchange nothing (PAPER.md:387)
+    elif nparts == 5:
+        assert dd.pulls[1] > 0 and dd.pulls[3] > 0
+    dd.close()
+    F = o.new_field()
+    o.run_mrab([F], nsteps, 0.0, 1, source_on=(True,))
+    share = np.array([np.linalg.norm(F.q[part == p]) for p in range(nparts)]) / np.linalg.norm(F.q)
+    assert share.min() > 0.02, share                                   # the wave has crossed every cut
+    assert rel_l2(q, F.q) < (1e-10 if precision == 64 else 1e-5), rel_l2(q, F.q)
+    g = make_gpu(cfg, precision)
+    g.dg_step(nsteps)
+    q1 = g.dg_get_fields()
+    g.close()
+    assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
+
+
 @pytest.mark.gpu
 def test_halo_and_spill_calls_reject_bad_arguments():
     """Error behaviour stated in include/dgrtm.h: wrong arguments come back as error codes (DGError), nothing aborts."""
@@ -121,26 +224,39 @@ def test_halo_and_spill_calls_reject_bad_arguments():
     cfg3 = make_config("cfg3_lts", hexes=(4, 4, 6), N=2)
     g = make_gpu(cfg3, 32)
     with pytest.raises(pk.DGError):
-        g.dg_get_trace_device()                                      # the halo exchange is single-rate
+        g.dg_get_trace_device()                                      # one buffer only for single-rate: dg_get_trace_levels
+    cur, half, n = g.dg_get_trace_levels()
+    assert len(cur) == 3 and half not in cur and n > 0
+    g.dg_step_fine(1)
+    with pytest.raises(pk.DGError):
+        g.dg_step(1)                                                 # inside a global step
+    g.dg_step_fine(3)
+    g.dg_step(1)
+    lev = g.dg_get_levels()
+    with pytest.raises(pk.DGError):
+        g.dg_set_model_levels(cfg3["rho"], cfg3["c"], 3, 1e-4, np.where(lev == 1, 3, lev))     # level out of range
+    with pytest.raises(pk.DGError):
+        g.dg_set_model_levels(cfg3["rho"], cfg3["c"], 3, 1e-4, np.where(lev == 1, 0, lev))     # neighbours two levels apart
     g.close()
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N,precision,world", [(3, 64, 2), (3, 32, 3)])
-def test_one_process_per_sub_domain(N, precision, world, tmp_path):
+@pytest.mark.parametrize("N,precision,world,workload", [(3, 64, 2, "cfg2_two_layer"), (3, 32, 3, "cfg2_two_layer"),
+                                                        (3, 64, 3, "cfg3_lts")])
+def test_one_process_per_sub_domain(N, precision, world, workload, tmp_path):
     """RankDecomposition: one process per sub-domain (gloo for the host side, CUDA IPC mappings of the neighbours'
     workspaces as the source of k_halo), all on cuda:0 here.  Same result as the single-domain run of the library."""
     import socket
     import torch.multiprocessing as mp
     import decomp_worker
-    nsteps, hexes = 60, (6, 5, 4)
+    nsteps, hexes = (60, (6, 5, 4)) if workload == "cfg2_two_layer" else (50, (6, 6, 8))   # cfg3_lts: three levels
     with socket.socket() as sk:
         sk.bind(("127.0.0.1", 0))
         port = sk.getsockname()[1]
     out = str(tmp_path / "q.npy")
-    mp.spawn(decomp_worker.run, args=(world, port, N, precision, nsteps, hexes, out), nprocs=world, join=True)
+    mp.spawn(decomp_worker.run, args=(world, port, N, precision, nsteps, hexes, out, workload), nprocs=world, join=True)
     q = np.load(out)
-    cfg = _cfg(hexes=hexes, N=N)
+    cfg = _cfg(hexes=hexes, N=N) if workload == "cfg2_two_layer" else _lts_cfg(N, hexes=hexes, nsteps=nsteps)
     g = make_gpu(cfg, precision)
     g.dg_step(nsteps)
     q1 = g.dg_get_fields()
