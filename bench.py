@@ -530,7 +530,9 @@ def extra_rtm_shot(torch, device, peak, peak_src, hexes, nsteps, traffic_table=N
 def extra_decomposition(torch, device, hexes, T=200):
     """Config 2 cut into 2 and 4 sub-domains that step in lock-step on this one GPU (decomp.py: halo fetch by k_halo from
     the neighbour's trace buffer, then one step per sub-domain): what the decomposition itself costs - smaller launches
-    and the halo kernels - before any NVLink is involved (one GPU in this pool)."""
+    and the halo kernels - before any NVLink is involved (one GPU in this pool).  Then the
+    multi-rate scheme on a three-level mesh: level weights, with and without the finest level kept off the cuts
+    (fetches per fine step of the cycle)."""
     from workloads import make_config
     from paper_1506_00907_b200.decomp import Decomposition, partition_elements
     cfg = make_config("cfg2_two_layer", hexes=hexes)
@@ -555,6 +557,38 @@ def extra_decomposition(torch, device, hexes, T=200):
         out.append({"sub_domains": nparts, "elements": [int(len(e)) for e in dd.elems], "halo_faces": int(halo),
                     "us_per_time_step": round(us, 2), "launches_per_time_step": (dd.launch_count() - n0) / T,
                     "value": 4 * dd.K * dd.Np / (us * 1e-6), "unit": UNIT})
+        dd.close()
+    # the multi-rate scheme on a three-level mesh of config 3's recipe: level weights, the finest level off the cuts
+    cfg = make_config("cfg3_lts", hexes=(32, 32, 16) if hexes is None else (8, 8, 8))
+    Tg = max(T // 4, 2)
+    for nparts, lump in ((1, False), (2, False), (2, True), (4, True)):
+        import paper_1506_00907_b200 as pk
+        g = pk.DG(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], default_bc=cfg["default_bc"])
+        g.dg_set_model(cfg["rho"], cfg["c"], cfg["nlevels"], cfg["cfl"])
+        level = g.dg_get_levels()
+        g.close()
+        finest = level == cfg["nlevels"] - 1
+        part = partition_elements(cfg["EToV"], cfg["VX"], nparts, 2.0 ** level, lump=finest if lump else None)
+        dd = Decomposition(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
+                           default_bc=cfg["default_bc"], cfl=cfg["cfl"], nlevels=cfg["nlevels"])
+        dd.bind_torch(device)
+        s = cfg["source"]
+        dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+        dd.dg_step(3)
+        torch.cuda.synchronize(device)
+        dd.pulls[:] = 0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        dd.dg_step(Tg)
+        e1.record()
+        torch.cuda.synchronize(device)
+        us = e0.elapsed_time(e1) * 1e3 / Tg
+        upd = float((np.bincount(level, minlength=cfg["nlevels"]) * 2 ** np.arange(cfg["nlevels"])).sum())   # element updates per global step
+        out.append({"workload": "cfg3_lts", "hexes": list(cfg["hexes"]), "levels": [int(x) for x in np.bincount(level)],
+                    "sub_domains": nparts, "finest_level_lumped": lump, "elements": [int(len(e)) for e in dd.elems],
+                    "work_per_sub_domain": [float((2.0 ** level[e]).sum()) for e in dd.elems],
+                    "halo_fetches_per_fine_step": [float(x) / Tg for x in dd.pulls],
+                    "us_per_global_step": round(us, 2), "value": 4 * upd * dd.Np / (us * 1e-6), "unit": UNIT})
         dd.close()
     return out
 
