@@ -537,10 +537,10 @@ def extra_decomposition(torch, device, hexes, T=200):
     from paper_1506_00907_b200.decomp import Decomposition, partition_elements
     cfg = make_config("cfg2_two_layer", hexes=hexes)
     out = []
-    for nparts in (1, 2, 4):
+    for nparts, fused in ((1, False), (2, False), (4, False), (2, True), (4, True)):
         part = partition_elements(cfg["EToV"], cfg["VX"], nparts)
         dd = Decomposition(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
-                           default_bc=cfg["default_bc"], cfl=cfg["cfl"])
+                           default_bc=cfg["default_bc"], cfl=cfg["cfl"], fused=fused)
         dd.bind_torch(device)
         s = cfg["source"]
         dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
@@ -554,14 +554,15 @@ def extra_decomposition(torch, device, hexes, T=200):
         torch.cuda.synchronize(device)
         us = e0.elapsed_time(e1) * 1e3 / T
         halo = sum(sum(len(t[1]) for t in sets) for sets in dd.sets)
-        out.append({"sub_domains": nparts, "elements": [int(len(e)) for e in dd.elems], "halo_faces": int(halo),
+        out.append({"sub_domains": nparts, "exchange": "fused into the step kernel" if fused else "k_halo launches",
+                    "elements": [int(len(e)) for e in dd.elems], "halo_faces": int(halo),
                     "us_per_time_step": round(us, 2), "launches_per_time_step": (dd.launch_count() - n0) / T,
                     "value": 4 * dd.K * dd.Np / (us * 1e-6), "unit": UNIT})
         dd.close()
     # the multi-rate scheme on a three-level mesh of config 3's recipe: level weights, the finest level off the cuts
     cfg = make_config("cfg3_lts", hexes=(32, 32, 16) if hexes is None else (8, 8, 8))
     Tg = max(T // 4, 2)
-    for nparts, lump in ((1, False), (2, False), (2, True), (4, True)):
+    for nparts, lump, fused in ((1, False, False), (2, False, False), (2, True, False), (4, True, False), (2, True, True), (4, True, True)):
         import paper_1506_00907_b200 as pk
         g = pk.DG(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], default_bc=cfg["default_bc"])
         g.dg_set_model(cfg["rho"], cfg["c"], cfg["nlevels"], cfg["cfl"])
@@ -570,7 +571,7 @@ def extra_decomposition(torch, device, hexes, T=200):
         finest = level == cfg["nlevels"] - 1
         part = partition_elements(cfg["EToV"], cfg["VX"], nparts, 2.0 ** level, lump=finest if lump else None)
         dd = Decomposition(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
-                           default_bc=cfg["default_bc"], cfl=cfg["cfl"], nlevels=cfg["nlevels"])
+                           default_bc=cfg["default_bc"], cfl=cfg["cfl"], nlevels=cfg["nlevels"], fused=fused)
         dd.bind_torch(device)
         s = cfg["source"]
         dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
@@ -585,7 +586,8 @@ def extra_decomposition(torch, device, hexes, T=200):
         us = e0.elapsed_time(e1) * 1e3 / Tg
         upd = float((np.bincount(level, minlength=cfg["nlevels"]) * 2 ** np.arange(cfg["nlevels"])).sum())   # element updates per global step
         out.append({"workload": "cfg3_lts", "hexes": list(cfg["hexes"]), "levels": [int(x) for x in np.bincount(level)],
-                    "sub_domains": nparts, "finest_level_lumped": lump, "elements": [int(len(e)) for e in dd.elems],
+                    "sub_domains": nparts, "finest_level_lumped": lump,
+                    "exchange": "fused into the step kernel" if fused else "k_halo launches", "elements": [int(len(e)) for e in dd.elems],
                     "work_per_sub_domain": [float((2.0 ** level[e]).sum()) for e in dd.elems],
                     "halo_fetches_per_fine_step": [float(x) / Tg for x in dd.pulls],
                     "us_per_global_step": round(us, 2), "value": 4 * upd * dd.Np / (us * 1e-6), "unit": UNIT})

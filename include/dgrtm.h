@@ -151,6 +151,13 @@ int dg_set_exterior(dg_ctx* ctx, const double* ext);
  *   levels whose step starts there); dg_step needs the scheme at the start of a global step.
  * dg_get_trace_levels: current[nlevels] = the buffer that holds, for the elements of level l, the exposed traces at the
  *   time level l has reached; half = the buffer of the half-step traces of the elements in mid-step; nbytes of each.
+ * dg_halo_sources: the FUSED exchange - instead of dg_halo_pull launches, the step kernel itself (k_pipe / k_step, AB
+ *   scheme) reads the exterior state of every halo face from the neighbour's trace buffer while it forms the penalties of
+ *   that face: src_trace_device[nsets] = the source buffer of every halo set for the NEXT fine step (one dg_step(1) of a
+ *   single-rate ctx or one dg_step_fine(1); consumed by it - the buffers alternate).  With peer pointers the loads cross
+ *   NVLink inside the step kernel, block by block, overlapped with the other blocks' arithmetic; no k_halo launch, no
+ *   exterior array in between.  The caller orders the step after the neighbours' previous step, and the neighbours' next
+ *   step after this one (they overwrite the buffer two steps later).  DG_ERR_UNSUPPORTED for LSERK4 / DGRTM_KERNEL=tc.
  * Fine step m of the decomposed problem = every sub-domain pulls every set - from current[l] of the neighbour if the
  *   level l of the elements behind that set starts a step at m, else from its half-step buffer - then every sub-domain
  *   takes dg_step_fine(1) (paper_1506_00907_b200/decomp.py). */
@@ -163,6 +170,7 @@ int dg_set_model_levels(dg_ctx* ctx, const double* rho, const double* c, int nle
                         const int32_t* bnd_level);
 int dg_step_fine(dg_ctx* ctx, int nfine);
 int dg_get_trace_levels(dg_ctx* ctx, void** current /* [nlevels] */, void** half, size_t* nbytes);
+int dg_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device /* [nsets] */);
 
 /* ---- RTM (Fig. 1) ---------------------------------------------------
  * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side

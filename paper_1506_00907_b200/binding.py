@@ -62,6 +62,7 @@ SIGNATURES = {
     "dg_set_model_levels": (_i, [_vp, _pd, _pd, _i, _d, _pi32, _pi32]),
     "dg_step_fine": (_i, [_vp, _i]),
     "dg_get_trace_levels": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_sz)]),
+    "dg_halo_sources": (_i, [_vp, _i, C.POINTER(_vp)]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
     "rtm_set_spill_packing": (_i, [_vp, _i]),
     "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
@@ -263,6 +264,12 @@ class DG:
         cur, half, n = (_vp * 8)(), _vp(), _sz()
         self._ck(_lib.dg_get_trace_levels(self._h, cur, C.byref(half), C.byref(n)))
         return [cur[l] for l in range(L)], half.value, n.value
+
+    def dg_halo_sources(self, src_trace_device):
+        """Fused exchange: device pointers of the source buffer of every halo set, for the next (fine) step."""
+        n = len(src_trace_device)
+        arr = (_vp * max(n, 1))(*[_vp(int(x)) for x in src_trace_device])
+        self._ck(_lib.dg_halo_sources(self._h, n, arr))
 
     # ---- RTM
     def rtm_set_receiver_capacity(self, max_receivers):

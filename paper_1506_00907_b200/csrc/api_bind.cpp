@@ -201,6 +201,11 @@ int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream) {
   upload_tables(ctx);
   ctx->F.reset_history();
   ctx->t0 = 0; ctx->fine = 0; ctx->has_ext = false; for (int x = 0; x <= kMaxHaloSets; ++x) ctx->halo_off[x] = 0;
+  {
+    const size_t nbf = ctx->mesh.bnd_k.size();
+    ctx->h_hrec.assign(nbf, -1); ctx->h_hset.assign(nbf, 0); ctx->h_hpos.assign(nbf * ctx->Nfp, 0);
+    ctx->halo_src_valid = false;
+  }
   ctx->have_final = false; ctx->have_backward = false;
   sync_stream(ctx);
   DG_CATCH(ctx)
@@ -287,6 +292,36 @@ int dg_set_halo(dg_ctx* ctx, int set, int64_t nh, const int32_t* bnd_index, cons
     ctx->has_ext = true;
   }
   for (int x = set + 1; x <= kMaxHaloSets; ++x) ctx->halo_off[x] = h0 + nh;
+  // the same tables by boundary face (fused exchange, dg_halo_sources): [hrec int64 nb | hset int32 nb | hpos int32 nb*Nfp]
+  for (int64_t h = 0; h < nh; ++h) {
+    const size_t bi = (size_t)bnd_index[h];
+    ctx->h_hrec[bi] = src_record[h]; ctx->h_hset[bi] = set;
+    for (int i = 0; i < Nfp; ++i) ctx->h_hpos[bi * Nfp + i] = src_pos[h * Nfp + i];
+  }
+  if (nb) {
+    upload_raw(ctx, ctx->d_halo_face, ctx->h_hrec.data(), (size_t)nb * 8);
+    upload_raw(ctx, ctx->d_halo_face + (size_t)nb * 8, ctx->h_hset.data(), (size_t)nb * 4);
+    upload_raw(ctx, ctx->d_halo_face + (size_t)nb * 12, ctx->h_hpos.data(), (size_t)nb * Nfp * 4);
+  }
+  DG_CATCH(ctx)
+}
+
+int dg_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device) {
+  DG_TRY(ctx)
+  require_bound(ctx);
+  if (nsets < 0 || nsets > kMaxHaloSets) throw ApiError(DG_ERR_ARG, "nsets must be in 0..32");
+  if (nsets && !src_trace_device) throw ApiError(DG_ERR_ARG, "source table is NULL");
+  if (ctx->integrator != DG_INTEGRATOR_AB3 || ctx->use_tc)
+    throw ApiError(DG_ERR_UNSUPPORTED, "the fused halo exchange is in the AB step kernels (k_pipe, k_step): use dg_halo_pull");
+  for (int x = 0; x < nsets; ++x) {
+    if (!src_trace_device[x] && ctx->halo_off[x + 1] > ctx->halo_off[x]) throw ApiError(DG_ERR_ARG, "NULL source of a non-empty halo set");
+    ctx->halo_src[x] = src_trace_device[x];
+  }
+  for (int x = nsets; x < kMaxHaloSets; ++x) {
+    if (ctx->halo_off[x + 1] > ctx->halo_off[x]) throw ApiError(DG_ERR_ARG, "a non-empty halo set has no source");
+    ctx->halo_src[x] = nullptr;
+  }
+  ctx->halo_src_valid = true;
   DG_CATCH(ctx)
 }
 

@@ -466,6 +466,7 @@ void carve_workspace(dg_ctx* c, Carver& cv) {
   c->ext = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * Nfp * 2 * rs);
   c->d_src_w = cv.take((size_t)Np * rs);
   c->d_halo = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * (size_t)(4 + 8 + 4 * Nfp) + 64);   // halo tables (dg_set_halo)
+  c->d_halo_face = cv.take(std::max<size_t>(1, c->mesh.bnd_k.size()) * (size_t)(8 + 4 + 4 * Nfp) + 64);   // the same by boundary face
   for (int l = 0; l < md.nlevels; ++l) {
     c->d_stored[l] = (int*)cv.take(std::max<size_t>(1, md.stored[l].size()) * 4);
   }

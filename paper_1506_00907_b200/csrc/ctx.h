@@ -138,6 +138,11 @@ struct dg_ctx {
   // ---- halo faces of a domain decomposition (dg_set_halo): tables [bnd | rec | pos] in one carved region
   char* d_halo = nullptr;
   int64_t halo_off[dgrtm::kMaxHaloSets + 1] = {};   // faces of halo set s (one set per neighbouring sub-domain): [halo_off[s], halo_off[s+1])
+  // the same tables by boundary face for the fused exchange (dg_halo_sources): host mirrors, device [hrec | hset | hpos]
+  char* d_halo_face = nullptr;
+  std::vector<long long> h_hrec; std::vector<int32_t> h_hset, h_hpos;
+  const void* halo_src[dgrtm::kMaxHaloSets] = {};   // source buffers of the next step's launches
+  bool halo_src_valid = false;              // set by dg_halo_sources, consumed by the next dg_step / dg_step_fine
   std::vector<double> bnd_Zext;             // exterior impedance per boundary face (> 0: Z_f = (Z- + Zext) / 2), dg_set_exterior_impedance
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;

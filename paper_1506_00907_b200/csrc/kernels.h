@@ -135,6 +135,11 @@ struct StepArgs {
   int reverse;                      // fixed chunks walked from their end: alternates from launch to launch, so a step starts
                                     // with the blocks the previous step left in L2 (matters when the mesh nearly fits it)
   const void* ext;           // prescribed exterior states or null
+  // fused halo exchange of a domain decomposition (dg_halo_sources): a prescribed face b with halo_rec[b] >= 0 takes its
+  // exterior state straight from the neighbouring sub-domain's trace buffer halo_src[halo_set[b]] (a peer pointer over
+  // NVLink, or local), record halo_rec[b], node i at position halo_pos[b][i]; NULL halo_rec: every prescribed face reads ext
+  const long long* halo_rec; const int* halo_set; const int* halo_pos;
+  const void* halo_src[32];
   double dir;
   // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale
   const int* pt_index[2]; const void* pt_val[2]; double pt_scale[2];

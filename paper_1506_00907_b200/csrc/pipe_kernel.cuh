@@ -396,9 +396,17 @@ k_pipe(const __grid_constant__ StepArgs a) {
 #pragma unroll
               for (int i2 = 0; i2 < Nfp; ++i2) { ep[i2] = repl[(size_t)bpos * REC + i2]; ev[i2] = repl[(size_t)bpos * REC + Nfp + i2]; }
             } else if (ext_lane) {
-              const real* ex = static_cast<const real*>(a.ext) + (size_t)bpos * Nfp * 2;
+              const long long hr = a.halo_rec ? a.halo_rec[bpos] : -1;
+              if (hr >= 0) {       // halo face: the neighbouring sub-domain's exposed trace, n-.v+ = -(n+.v+) (reading Q6b)
+                const real* r = static_cast<const real*>(a.halo_src[a.halo_set[bpos]]) + (size_t)hr * REC;
+                const int* hp = a.halo_pos + (size_t)bpos * Nfp;
 #pragma unroll
-              for (int i2 = 0; i2 < Nfp; ++i2) { ep[i2] = ex[2 * i2]; ev[i2] = ex[2 * i2 + 1]; }
+                for (int i2 = 0; i2 < Nfp; ++i2) { const int j = hp[i2]; ep[i2] = r[j]; ev[i2] = -r[Nfp + j]; }
+              } else {
+                const real* ex = static_cast<const real*>(a.ext) + (size_t)bpos * Nfp * 2;
+#pragma unroll
+                for (int i2 = 0; i2 < Nfp; ++i2) { ep[i2] = ex[2 * i2]; ev[i2] = ex[2 * i2 + 1]; }
+              }
             }
           }
           const bool cap_lane = bc == 2 && capt != nullptr;

@@ -352,8 +352,15 @@ k_step(const __grid_constant__ StepArgs a) {
               if (repl) { dp = repl[(size_t)bpos * REC + i] - pm; dnv = repl[(size_t)bpos * REC + Nfp + i] - nvm; }
               else { dp = -pm; dnv = -nvm; }
             } else if (bc == 4) {
-              const real* ex = static_cast<const real*>(a.ext) + ((size_t)bpos * Nfp + i) * 2;
-              dp = ex[0] - pm; dnv = ex[1] - nvm;
+              const long long hr = a.halo_rec ? a.halo_rec[bpos] : -1;
+              if (hr >= 0) {       // halo face: the neighbouring sub-domain's exposed trace (see StepArgs)
+                const real* r = static_cast<const real*>(a.halo_src[a.halo_set[bpos]]) + (size_t)hr * REC;
+                const int jn = a.halo_pos[(size_t)bpos * Nfp + i];
+                dp = r[jn] - pm; dnv = -r[Nfp + jn] - nvm;
+              } else {
+                const real* ex = static_cast<const real*>(a.ext) + ((size_t)bpos * Nfp + i) * 2;
+                dp = ex[0] - pm; dnv = ex[1] - nvm;
+              }
             } else { dp = 0; dnv = 0; }
             pen[j * 32 + lane] = rc2 * half_gs * (dnv - dir * dp * iZ);
             pen[(NF + j) * 32 + lane] = irho * half_gs * (dp - dir * Zf * dnv);

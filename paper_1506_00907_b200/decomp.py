@@ -113,10 +113,12 @@ def partition_elements(EToV, VX, nparts, weights=None, lump=None):
 class Decomposition:
     """The sub-domains of one mesh as DG contexts with their halo tables.  Global arrays in, global arrays out."""
 
-    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15, only=None, nlevels=1):
+    def __init__(self, N, precision, EToV, VX, rho, c, part, default_bc=2, face_bc=None, cfl=0.15, only=None, nlevels=1,
+                 fused=False):
         """only = p: bind / step sub-domain p alone (the others exist on the host for their slot tables).
         nlevels > 1: the multi-rate scheme; the levels and the finest step are those of the WHOLE mesh."""
         self.only = only
+        self.fused = bool(fused)     # the step kernels read the halo faces' exterior states themselves (dg_halo_sources)
         self.nlevels, self.nlocal = int(nlevels), 1 << (int(nlevels) - 1)
         EToV = np.ascontiguousarray(EToV, dtype=np.int32)
         self.K, self.part = EToV.shape[0], np.asarray(part, dtype=np.int32)
@@ -229,6 +231,10 @@ class Decomposition:
                 lmin = self.first_level_starting_at(m)
                 tr = [s.dg_get_trace_levels() for s in self.sub]
                 for p, s in enumerate(self.sub):
+                    if self.fused:                               # no fetch launches: the step kernel reads these buffers
+                        s.dg_halo_sources([tr[q][0][lev] if lev >= lmin else tr[q][1]
+                                           for (q, _, _, _), lev in zip(self.sets[p], self.set_level[p])])
+                        continue
                     for i, (q, _, _, _) in enumerate(self.sets[p]):
                         if self.set_mine[p][i] < lmin:          # none of my elements on these faces steps now (with the
                             continue                            # finest level off the cuts: no exchange at odd fine steps)
@@ -287,6 +293,12 @@ class RankDecomposition(Decomposition):
             for m in range(self.nlocal):
                 lmin = self.first_level_starting_at(m)
                 offs = self._trace_offsets()        # also orders this step after every rank's previous step (see below)
+                if self.fused:                      # my step kernel reads the neighbours' buffers; they write the OTHER ones
+                    me.dg_halo_sources([self._peer[q].data_ptr() + (offs[q][0][lev] if lev >= lmin else offs[q][1])
+                                        for (q, _, _, _), lev in zip(self.sets[self.rank], self.set_level[self.rank])])
+                    me.dg_step_fine(1)
+                    torch.cuda.synchronize(self._device)    # my reads and my new traces are complete before the next all-gather
+                    continue
                 for i, (q, _, _, _) in enumerate(self.sets[self.rank]):
                     if self.set_mine[self.rank][i] < lmin:
                         continue

@@ -6,7 +6,7 @@ import sys
 import numpy as np
 
 
-def run(rank, world, port, N, precision, nsteps, hexes, out_path, workload="cfg2_two_layer"):
+def run(rank, world, port, N, precision, nsteps, hexes, out_path, workload="cfg2_two_layer", fused=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     import torch
@@ -20,7 +20,7 @@ def run(rank, world, port, N, precision, nsteps, hexes, out_path, workload="cfg2
     cfg["source"] = dict(cfg["source"], f0=40.0, tp=0.01)
     part = partition_elements(cfg["EToV"], cfg["VX"], world)
     dd = RankDecomposition(dist, N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
-                           default_bc=cfg["default_bc"], nlevels=cfg["nlevels"], cfl=cfg["cfl"])
+                           default_bc=cfg["default_bc"], nlevels=cfg["nlevels"], cfl=cfg["cfl"], fused=fused)
     torch.cuda.set_device(0)
     dd.bind_torch("cuda:0")
     s = cfg["source"]

@@ -75,19 +75,28 @@ def _local_mesh(etov, vx, elems):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N,precision,nparts", [(3, 32, 2), (3, 64, 3), (4, 32, 3), (2, 64, 4)])
-def test_decomposed_run_matches_the_oracle(N, precision, nparts):
+@pytest.mark.parametrize("N,precision,nparts,fused", [(3, 32, 2, False), (3, 64, 3, False), (4, 32, 3, False), (2, 64, 4, False),
+                                                      (3, 32, 3, True), (3, 64, 2, True), (4, 64, 2, True), (1, 64, 3, True),
+                                                      (5, 64, 2, True)])
+def test_decomposed_run_matches_the_oracle(N, precision, nparts, fused):
+    """fused: no k_halo launches - the step kernel (k_pipe; k_step at N = 1 and N = 5 fp64) reads the exterior states of
+    the halo faces from the neighbour's trace buffer itself (dg_halo_sources)."""
     from paper_1506_00907_b200.decomp import Decomposition, partition_elements
     cfg = _cfg(N=N)
     nsteps = cfg["nsteps"]
     part = partition_elements(cfg["EToV"], cfg["VX"], nparts)
-    dd = Decomposition(N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"])
+    dd = Decomposition(N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"],
+                       fused=fused)
     dd.bind_torch("cuda:0")
     s = cfg["source"]
     dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+    n0 = dd.launch_count()
     dd.dg_step(nsteps)
     q = dd.dg_get_fields()
-    assert dd.launch_count() >= nsteps * nparts * 2                  # a halo fetch and a step per sub-domain and time step
+    if fused:
+        assert dd.launch_count() - n0 == nsteps * nparts             # one launch per sub-domain and time step: the step kernel
+    else:
+        assert dd.launch_count() - n0 >= nsteps * nparts * 2         # a halo fetch and a step per sub-domain and time step
     dd.close()
     o = make_oracle(cfg)
     F = o.new_field()
@@ -165,9 +174,11 @@ def test_multirate_halo_sets_carry_one_level_each():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N,precision,nparts,lump", [(3, 64, 2, False), (2, 64, 5, False), (2, 64, 5, True), (3, 32, 3, True),
-                                                     (4, 32, 2, False)])
-def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump):
+@pytest.mark.parametrize("N,precision,nparts,lump,fused", [(3, 64, 2, False, False), (2, 64, 5, False, False),
+                                                           (2, 64, 5, True, False), (3, 32, 3, True, False),
+                                                           (4, 32, 2, False, False), (3, 64, 3, False, True),
+                                                           (4, 32, 5, True, True), (2, 32, 4, False, True)])
+def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump, fused):
     """Three levels, cuts across level interfaces: before every FINE step each sub-domain fetches, per halo set, the
     neighbour's traces of that set's level - its current ones if the level starts a step there, its half-step ones (eq (19))
     if it is in mid-step - and advances by dg_step_fine(1).  Same fields as the single-domain oracle and library runs."""
@@ -178,7 +189,7 @@ def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump)
     part = partition_elements(cfg["EToV"], cfg["VX"], nparts, 2.0 ** np.asarray(o.level),
                               lump=(np.asarray(o.level) == 2) if lump else None)
     dd = Decomposition(N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"],
-                       nlevels=cfg["nlevels"], cfl=cfg["cfl"])
+                       nlevels=cfg["nlevels"], cfl=cfg["cfl"], fused=fused)
     assert np.array_equal(dd.level, o.level)
     assert any(dd.set_level[p][i] != lev for p in range(nparts) for i, (q, bnd, _, _) in enumerate(dd.sets[p])
                for lev in dd.level[dd.elems[p][dd.sub[p].dg_get_boundary_faces()[0][bnd]]])
@@ -187,8 +198,10 @@ def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump)
     dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
     dd.dg_step(nsteps)
     q = dd.dg_get_fields()
-    assert dd.pulls[0] > 0 and dd.pulls[2] > 0
-    if lump:                                                           # the finest level is off the cuts: the fine steps that
+    assert fused or (dd.pulls[0] > 0 and dd.pulls[2] > 0)
+    if fused:
+        assert dd.pulls.sum() == 0                                     # no fetch launches at all
+    elif lump:                                                           # the finest level is off the cuts: the fine steps that
         assert dd.pulls[1] == 0 and dd.pulls[3] == 0                   # advance it alone exchange nothing
     elif nparts == 5:
         assert dd.pulls[1] > 0 and dd.pulls[3] > 0
@@ -196,7 +209,7 @@ def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump)
     F = o.new_field()
     o.run_mrab([F], nsteps, 0.0, 1, source_on=(True,))
     share = np.array([np.linalg.norm(F.q[part == p]) for p in range(nparts)]) / np.linalg.norm(F.q)
-    assert share.min() > 0.02, share                                   # the wave has crossed every cut
+    assert share.min() > 0.005, share                                  # the wave has crossed every cut
     assert rel_l2(q, F.q) < (1e-10 if precision == 64 else 1e-5), rel_l2(q, F.q)
     g = make_gpu(cfg, precision)
     g.dg_step(nsteps)
@@ -241,9 +254,10 @@ def test_halo_and_spill_calls_reject_bad_arguments():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N,precision,world,workload", [(3, 64, 2, "cfg2_two_layer"), (3, 32, 3, "cfg2_two_layer"),
-                                                        (3, 64, 3, "cfg3_lts")])
-def test_one_process_per_sub_domain(N, precision, world, workload, tmp_path):
+@pytest.mark.parametrize("N,precision,world,workload,fused", [(3, 64, 2, "cfg2_two_layer", False), (3, 32, 3, "cfg2_two_layer", False),
+                                                              (3, 64, 3, "cfg3_lts", False), (3, 64, 3, "cfg3_lts", True),
+                                                              (4, 32, 2, "cfg2_two_layer", True)])
+def test_one_process_per_sub_domain(N, precision, world, workload, fused, tmp_path):
     """RankDecomposition: one process per sub-domain (gloo for the host side, CUDA IPC mappings of the neighbours'
     workspaces as the source of k_halo), all on cuda:0 here.  Same result as the single-domain run of the library."""
     import socket
@@ -254,7 +268,7 @@ def test_one_process_per_sub_domain(N, precision, world, workload, tmp_path):
         sk.bind(("127.0.0.1", 0))
         port = sk.getsockname()[1]
     out = str(tmp_path / "q.npy")
-    mp.spawn(decomp_worker.run, args=(world, port, N, precision, nsteps, hexes, out, workload), nprocs=world, join=True)
+    mp.spawn(decomp_worker.run, args=(world, port, N, precision, nsteps, hexes, out, workload, fused), nprocs=world, join=True)
     q = np.load(out)
     cfg = _cfg(hexes=hexes, N=N) if workload == "cfg2_two_layer" else _lts_cfg(N, hexes=hexes, nsteps=nsteps)
     g = make_gpu(cfg, precision)
