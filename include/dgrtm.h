@@ -211,6 +211,21 @@ int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out);
  * (PAPER.md:460).  Images of successive shots add up.  Synchronises. */
 int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double updir[3],
                       int imaging, int64_t first_image_step);
+/* A phase of a shot in PARTS - for a domain decomposition, where the sub-domains exchange halo traces between the fine
+ * steps ("for the backward run ... both source and receivers simulations are performed using the same mesh
+ * partition", so the imaging condition needs no exchange): fine steps [fine0, fine0 + nfine) of a phase of nsteps global
+ * steps.  The part with fine0 = 0 initialises the phase exactly as the _shot call does (data / updir / imaging are read
+ * then and on every part; data may be NULL after the first), the part that reaches nsteps * 2^(L-1) finishes it (final
+ * capture and sample, data_out; earlier parts ignore data_out and do not synchronise).  An empty part at 0 (nfine = 0)
+ * initialises alone - the trace buffers can then be asked for before the first step.  The parts follow one another
+ * (DG_ERR_STATE otherwise).  rtm_forward_shot(n, d) = rtm_forward_part(n, 0, n * 2^(L-1), d), likewise backward.
+ * rtm_get_trace_levels: dg_get_trace_levels for field 0 (source wavefield) or 1 (receiver wavefield).
+ * rtm_halo_sources: dg_halo_sources for the receiver wavefield; a two-field step needs both, each for ONE fine step. */
+int rtm_forward_part(dg_ctx* ctx, int nsteps, int64_t fine0, int64_t nfine, double* data_out);
+int rtm_backward_part(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
+                      int64_t first_image_step, int64_t fine0, int64_t nfine);
+int rtm_get_trace_levels(dg_ctx* ctx, int field, void** current /* [nlevels] */, void** half, size_t* nbytes);
+int rtm_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device /* [nsets] */);
 int rtm_image_read(dg_ctx* ctx, double* I_out /* [K][Np] */);
 int rtm_image_zero(dg_ctx* ctx);
 /* Device address and size of the image in the library's blocked layout [block][Np][32] (device precision), inside the

@@ -71,6 +71,10 @@ SIGNATURES = {
     "rtm_bind_history": (_i, [_vp, _vp, _sz]),
     "rtm_forward_shot": (_i, [_vp, _i, _pd]),
     "rtm_backward_shot": (_i, [_vp, _i, _pd, _pd, _i, _i64]),
+    "rtm_forward_part": (_i, [_vp, _i, _i64, _i64, _pd]),
+    "rtm_backward_part": (_i, [_vp, _i, _pd, _pd, _i, _i64, _i64, _i64]),
+    "rtm_get_trace_levels": (_i, [_vp, _i, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_sz)]),
+    "rtm_halo_sources": (_i, [_vp, _i, C.POINTER(_vp)]),
     "rtm_image_read": (_i, [_vp, _pd]),
     "rtm_image_zero": (_i, [_vp]),
     "rtm_image_device": (_i, [_vp, C.POINTER(_vp), _psz]),
@@ -323,6 +327,32 @@ class DG:
         u = _f64(updir)
         self._ck(_lib.rtm_backward_shot(self._h, int(nsteps), _ptr(d, _pd), _ptr(u, _pd), int(imaging),
                                         int(first_image_step)))
+
+    def rtm_forward_part(self, nsteps, fine0, nfine, want_data=True):
+        """Fine steps [fine0, fine0 + nfine) of the forward phase; the recorded signals come back with the last part."""
+        nloc = self.dg_get_dt()[1]
+        last = fine0 + nfine == nsteps * nloc
+        data = np.empty((self.nr, nsteps * nloc + 1)) if (want_data and self.nr and last) else None
+        self._ck(_lib.rtm_forward_part(self._h, int(nsteps), int(fine0), int(nfine), _ptr(data, _pd)))
+        return data
+
+    def rtm_backward_part(self, nsteps, data, fine0, nfine, updir=(0.0, 0.0, -1.0), imaging=DG_IMAGING_CHARACTERISTIC,
+                          first_image_step=0):
+        d = None if data is None else _f64(data)
+        u = _f64(updir)
+        self._ck(_lib.rtm_backward_part(self._h, int(nsteps), _ptr(d, _pd), _ptr(u, _pd), int(imaging),
+                                        int(first_image_step), int(fine0), int(nfine)))
+
+    def rtm_get_trace_levels(self, field):
+        L = int(self.dg_get_dt()[1]).bit_length()
+        cur, half, n = (_vp * 8)(), _vp(), _sz()
+        self._ck(_lib.rtm_get_trace_levels(self._h, int(field), cur, C.byref(half), C.byref(n)))
+        return [cur[l] for l in range(L)], half.value, n.value
+
+    def rtm_halo_sources(self, src_trace_device):
+        n = len(src_trace_device)
+        arr = (_vp * max(n, 1))(*[_vp(int(x)) for x in src_trace_device])
+        self._ck(_lib.rtm_halo_sources(self._h, n, arr))
 
     def rtm_image_read(self):
         out = np.empty((self.K, self.Np))

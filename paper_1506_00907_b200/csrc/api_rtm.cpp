@@ -340,47 +340,69 @@ int rtm_bind_history(dg_ctx* ctx, void* dptr, size_t n) {
   DG_CATCH(ctx)
 }
 
-int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out) {
-  DG_TRY(ctx)
+// A phase of a shot in parts (rtm_forward_part / rtm_backward_part, include/dgrtm.h): fine steps [fine0, fine0 + nfine) of
+// the phase; the part that starts at 0 initialises the phase, the part that reaches its end finishes it.
+static void forward_part(dg_ctx* ctx, int nsteps, int64_t fine0, int64_t nfine, double* data_out) {
   require_history(ctx);
   if (nsteps < 1 || nsteps > ctx->hist_nsteps) throw ApiError(DG_ERR_NOMEM, "nsteps exceeds the bound history capacity (" + std::to_string(ctx->hist_nsteps) + ")");
   if (ctx->integrator != DG_INTEGRATOR_AB3) throw ApiError(DG_ERR_UNSUPPORTED, "RTM uses the AB3 / multi-rate AB3 integrator");
-  clear_field(ctx, ctx->F);
-  ctx->t0 = 0; ctx->fine = 0;
+  const int64_t total = (int64_t)nsteps * ctx->nlocal;
+  if (fine0 < 0 || nfine < 0 || fine0 + nfine > total) throw ApiError(DG_ERR_ARG, "fine steps outside the forward phase");
+  if (fine0 == 0 && !(ctx->part_phase == 1 && ctx->part_nsteps == nsteps && ctx->part_fresh)) {   // (an empty first part
+    clear_field(ctx, ctx->F);                                // initialises alone, so that the trace buffers can be asked for)
+    ctx->t0 = 0; ctx->fine = 0;
+    ctx->have_final = false; ctx->have_backward = false;
+    ctx->part_phase = 1; ctx->part_nsteps = nsteps; ctx->part_fresh = true;
+  } else if (ctx->part_phase != 1 || ctx->part_nsteps != nsteps || ctx->fine != fine0) {
+    throw ApiError(DG_ERR_STATE, "the parts of a forward phase follow one another from fine step 0");
+  }
   RunOpts o;
   o.direction = 1; o.fields[0] = &ctx->F; o.nfields = 1; o.source_on[0] = ctx->has_src;
-  o.capture = true; o.record = ctx->nr > 0; o.first_fine = 0; o.t0 = 0;
-  run_mrab(ctx, nsteps, o);
-  ctx->fine = (int64_t)nsteps * ctx->nlocal;
-  cuda_check(cudaMemcpyAsync(ctx->qfinal, ctx->F.q, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "save final state");
+  o.capture = true; o.record = ctx->nr > 0;
+  o.first_fine = fine0; o.t0 = (double)fine0 * ctx->dt_local;
+  o.fine_phase = fine0 % ctx->nlocal; o.nfine = nfine; o.finish = fine0 + nfine == total;
+  run_mrab(ctx, 0, o);
+  ctx->fine = fine0 + nfine;
+  if (nfine > 0) ctx->part_fresh = false;
+  if (o.finish) {
+    cuda_check(cudaMemcpyAsync(ctx->qfinal, ctx->F.q, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "save final state");
+    ctx->have_final = true; ctx->final_nsteps = nsteps;
+    ctx->data_valid = ctx->nr > 0;
+    ctx->part_phase = 0;
+  }
   check_launches(ctx);
-  ctx->have_final = true; ctx->final_nsteps = nsteps; ctx->have_backward = false;
-  ctx->data_valid = ctx->nr > 0;
-  if (data_out) copy_data(ctx, data_out, nullptr, (int64_t)nsteps * ctx->nlocal + 1);
-  sync_stream(ctx);
-  if (ctx->spill_window > 0) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
-  DG_CATCH(ctx)
+  if (o.finish) {
+    if (data_out) copy_data(ctx, data_out, nullptr, total + 1);
+    sync_stream(ctx);
+    if (ctx->spill_window > 0) cuda_check(cudaStreamSynchronize(ctx->copy_stream), "cudaStreamSynchronize (trace spill)");
+  }
 }
 
-int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
-                      int64_t first_image_step) {
-  DG_TRY(ctx)
+static void backward_part(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
+                          int64_t first_image_step, int64_t fine0, int64_t nfine) {
   require_history(ctx);
   if (!ctx->have_final) throw ApiError(DG_ERR_STATE, "rtm_forward_shot first");
   if (nsteps < 1 || nsteps > ctx->final_nsteps) throw ApiError(DG_ERR_ARG, "nsteps must be in 1..(steps of the forward shot)");
   if (!updir) throw ApiError(DG_ERR_ARG, "updir is NULL");
   if (imaging < 0 || imaging > 3) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
-  const int64_t ntot = ctx->final_nsteps;
-  if (!data && ctx->nr > 0 && !ctx->data_valid)
-    throw ApiError(DG_ERR_STATE, "the signals on the device belong to another receiver set: pass data");
-  if (data) ctx->data_valid = true;
-  if (data) copy_data(ctx, nullptr, data, ntot * ctx->nlocal + 1);   // NULL: the signals recorded on the device
-  // source field: restart from q(t_f) (history restarts, reading Q7); receiver field: from rest
-  cuda_check(cudaMemcpyAsync(ctx->F.q, ctx->qfinal, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "restore final state");
-  for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(ctx->F.hist[s], 0, field_bytes(ctx), ctx->stream), "memset hist");
-  ctx->F.reset_history();
-  refresh_traces(ctx, ctx->F);
-  clear_field(ctx, ctx->R);
+  const int64_t ntot = ctx->final_nsteps, total = (int64_t)nsteps * ctx->nlocal;
+  if (fine0 < 0 || nfine < 0 || fine0 + nfine > total) throw ApiError(DG_ERR_ARG, "fine steps outside the backward phase");
+  if (fine0 == 0 && !(ctx->part_phase == 2 && ctx->part_nsteps == nsteps && ctx->part_fresh)) {
+    if (!data && ctx->nr > 0 && !ctx->data_valid)
+      throw ApiError(DG_ERR_STATE, "the signals on the device belong to another receiver set: pass data");
+    if (data) ctx->data_valid = true;
+    if (data) copy_data(ctx, nullptr, data, ntot * ctx->nlocal + 1);   // NULL: the signals recorded on the device
+    // source field: restart from q(t_f) (history restarts, reading Q7); receiver field: from rest
+    cuda_check(cudaMemcpyAsync(ctx->F.q, ctx->qfinal, field_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream), "restore final state");
+    for (int s = 0; s < 3; ++s) cuda_check(cudaMemsetAsync(ctx->F.hist[s], 0, field_bytes(ctx), ctx->stream), "memset hist");
+    ctx->F.reset_history();
+    refresh_traces(ctx, ctx->F);
+    clear_field(ctx, ctx->R);
+    ctx->part_phase = 2; ctx->part_nsteps = nsteps; ctx->part_fresh = true;
+    ctx->fine = ntot * ctx->nlocal;
+  } else if (ctx->part_phase != 2 || ctx->part_nsteps != nsteps || ctx->fine != ntot * ctx->nlocal - fine0) {
+    throw ApiError(DG_ERR_STATE, "the parts of a backward phase follow one another from fine step 0");
+  }
   RunOpts o;
   o.direction = -1; o.fields[0] = &ctx->F; o.fields[1] = &ctx->R; o.nfields = 2;
   o.source_on[0] = ctx->has_src; o.source_on[1] = false;
@@ -388,13 +410,65 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
   o.image = true; o.imaging = imaging;
   for (int d = 0; d < 3; ++d) o.updir[d] = updir[d];
   o.image_min_fine = first_image_step * ctx->nlocal;
-  o.first_fine = ntot * ctx->nlocal;
-  o.t0 = (double)ntot * ((double)ctx->nlocal * ctx->dt_local);
-  run_mrab(ctx, nsteps, o);
-  ctx->fine = (ntot - nsteps) * ctx->nlocal;
+  o.first_fine = ntot * ctx->nlocal - fine0;
+  o.t0 = (double)o.first_fine * ctx->dt_local;
+  o.fine_phase = fine0 % ctx->nlocal; o.nfine = nfine; o.finish = fine0 + nfine == total;
+  run_mrab(ctx, 0, o);
+  ctx->fine = o.first_fine - nfine;
+  if (nfine > 0) ctx->part_fresh = false;
   check_launches(ctx);
-  ctx->have_backward = true;
-  sync_stream(ctx);
+  if (o.finish) { ctx->have_backward = true; ctx->part_phase = 0; sync_stream(ctx); }
+}
+
+int rtm_forward_shot(dg_ctx* ctx, int nsteps, double* data_out) {
+  DG_TRY(ctx)
+  forward_part(ctx, nsteps, 0, (int64_t)nsteps * ctx->nlocal, data_out);
+  DG_CATCH(ctx)
+}
+
+int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
+                      int64_t first_image_step) {
+  DG_TRY(ctx)
+  backward_part(ctx, nsteps, data, updir, imaging, first_image_step, 0, (int64_t)nsteps * ctx->nlocal);
+  DG_CATCH(ctx)
+}
+
+int rtm_forward_part(dg_ctx* ctx, int nsteps, int64_t fine0, int64_t nfine, double* data_out) {
+  DG_TRY(ctx)
+  forward_part(ctx, nsteps, fine0, nfine, data_out);
+  DG_CATCH(ctx)
+}
+
+int rtm_backward_part(dg_ctx* ctx, int nsteps, const double* data, const double updir[3], int imaging,
+                      int64_t first_image_step, int64_t fine0, int64_t nfine) {
+  DG_TRY(ctx)
+  backward_part(ctx, nsteps, data, updir, imaging, first_image_step, fine0, nfine);
+  DG_CATCH(ctx)
+}
+
+int rtm_get_trace_levels(dg_ctx* ctx, int field, void** current, void** half, size_t* nbytes) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (field != 0 && field != 1) throw ApiError(DG_ERR_ARG, "field must be 0 (source) or 1 (receivers)");
+  if (!current || !half || !nbytes) throw ApiError(DG_ERR_ARG, "current / half / nbytes is NULL");
+  Field& F = field == 0 ? ctx->F : ctx->R;
+  for (int l = 0; l < ctx->model.nlevels; ++l) current[l] = F.qfb[F.par[l]];
+  *half = F.qfh;
+  *nbytes = trace_bytes(ctx);
+  DG_CATCH(ctx)
+}
+
+int rtm_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device) {
+  DG_TRY(ctx)
+  require_history(ctx);
+  if (nsets < 0 || nsets > kMaxHaloSets) throw ApiError(DG_ERR_ARG, "nsets must be in 0..32");
+  if (nsets && !src_trace_device) throw ApiError(DG_ERR_ARG, "source table is NULL");
+  for (int x = 0; x < kMaxHaloSets; ++x) {
+    const void* p = x < nsets ? src_trace_device[x] : nullptr;
+    if (!p && ctx->halo_off[x + 1] > ctx->halo_off[x]) throw ApiError(DG_ERR_ARG, "a non-empty halo set has no source");
+    ctx->halo_src2[x] = p;
+  }
+  ctx->halo_src2_valid = true;
   DG_CATCH(ctx)
 }
 

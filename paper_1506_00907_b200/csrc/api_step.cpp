@@ -75,7 +75,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
   a.nfields = o.nfields; a.nlevels = L;
   a.geo = c->geo; a.nbr = c->nbr; a.wperm = c->wperm; a.blkflag = c->d_blkflag;
   a.ext = c->has_ext ? c->ext : nullptr;
-  if (c->halo_src_valid && o.nfields == 1) {   // fused halo exchange: this call's launches read the neighbours' buffers
+  if (c->halo_src_valid) {   // fused halo exchange: this call's launches read the neighbours' buffers
     if ((o.nfine >= 0 ? o.nfine : (int64_t)nglobal * nloc) != 1)
       throw ApiError(DG_ERR_STATE, "dg_halo_sources serves ONE fine step (the trace buffers alternate): dg_step(1) single-rate, dg_step_fine(1)");
     const size_t nbf = c->mesh.bnd_k.size();
@@ -83,6 +83,11 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     a.halo_set = reinterpret_cast<const int*>(c->d_halo_face + nbf * 8);
     a.halo_pos = reinterpret_cast<const int*>(c->d_halo_face + nbf * 12);
     for (int x = 0; x < kMaxHaloSets; ++x) a.halo_src[x] = c->halo_src[x];
+    if (o.nfields == 2) {
+      if (!c->halo_src2_valid) throw ApiError(DG_ERR_STATE, "two wavefields: rtm_halo_sources must name the receiver field's sources too");
+      for (int x = 0; x < kMaxHaloSets; ++x) a.halo_src2[x] = c->halo_src2[x];
+    }
+    c->halo_src2_valid = false;
     c->halo_src_valid = false;                 // the buffers alternate: sources are good for the step they were given for
   }
   a.sched = sched_counters(c);
@@ -161,6 +166,7 @@ void run_mrab(dg_ctx* c, int nglobal, const RunOpts& o) {
     }
   }
   const int64_t jend = o.first_fine + dir * nfine;
+  if (!o.finish) return;
   if (o.capture) {
     for (int l = 0; l < L; ++l) {
       if (md.stored[l].empty()) continue;

@@ -143,6 +143,10 @@ struct dg_ctx {
   std::vector<long long> h_hrec; std::vector<int32_t> h_hset, h_hpos;
   const void* halo_src[dgrtm::kMaxHaloSets] = {};   // source buffers of the next step's launches
   bool halo_src_valid = false;              // set by dg_halo_sources, consumed by the next dg_step / dg_step_fine
+  const void* halo_src2[dgrtm::kMaxHaloSets] = {};  // the same for the receiver wavefield (rtm_halo_sources)
+  bool halo_src2_valid = false;
+  bool part_fresh = false;                  // the phase is initialised and no fine step of it has run
+  int part_phase = 0, part_nsteps = 0;      // rtm_forward_part / rtm_backward_part: phase in progress (1 forward, 2 backward), its global steps
   std::vector<double> bnd_Zext;             // exterior impedance per boundary face (> 0: Z_f = (Z- + Zext) / 2), dg_set_exterior_impedance
   int* d_stored[dgrtm::kMaxLevels];         // per level: slot*4+f of the stored boundary faces
   double t0 = 0;
@@ -249,6 +253,7 @@ struct RunOpts {
   bool source_on[2] = {false, false};
   bool capture = false, replay = false, record = false;
   int inject_field = -1;
+  bool finish = true;                        // the run reaches the end of the phase: final capture / final receiver sample
   int64_t fine_phase = 0, nfine = -1;        // dg_step_fine: fine index within the cycle at the start, fine steps to run (-1: whole global steps)
   bool image = false;
   int imaging = DG_IMAGING_CHARACTERISTIC;

@@ -140,6 +140,7 @@ struct StepArgs {
   // NVLink, or local), record halo_rec[b], node i at position halo_pos[b][i]; NULL halo_rec: every prescribed face reads ext
   const long long* halo_rec; const int* halo_set; const int* halo_pos;
   const void* halo_src[32];
+  const void* halo_src2[32];   // the same for field 1 (backward phase: the receiver wavefield of the neighbouring sub-domain)
   double dir;
   // point terms (eq (15)): per field a per-slot row index (-1: none) into pt_val[row][Np], times pt_scale
   const int* pt_index[2]; const void* pt_val[2]; double pt_scale[2];

@@ -398,7 +398,7 @@ k_pipe(const __grid_constant__ StepArgs a) {
             } else if (ext_lane) {
               const long long hr = a.halo_rec ? a.halo_rec[bpos] : -1;
               if (hr >= 0) {       // halo face: the neighbouring sub-domain's exposed trace, n-.v+ = -(n+.v+) (reading Q6b)
-                const real* r = static_cast<const real*>(a.halo_src[a.halo_set[bpos]]) + (size_t)hr * REC;
+                const real* r = static_cast<const real*>((fi == 0 ? a.halo_src : a.halo_src2)[a.halo_set[bpos]]) + (size_t)hr * REC;
                 const int* hp = a.halo_pos + (size_t)bpos * Nfp;
 #pragma unroll
                 for (int i2 = 0; i2 < Nfp; ++i2) { const int j = hp[i2]; ep[i2] = r[j]; ev[i2] = -r[Nfp + j]; }

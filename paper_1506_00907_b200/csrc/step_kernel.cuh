@@ -354,7 +354,7 @@ k_step(const __grid_constant__ StepArgs a) {
             } else if (bc == 4) {
               const long long hr = a.halo_rec ? a.halo_rec[bpos] : -1;
               if (hr >= 0) {       // halo face: the neighbouring sub-domain's exposed trace (see StepArgs)
-                const real* r = static_cast<const real*>(a.halo_src[a.halo_set[bpos]]) + (size_t)hr * REC;
+                const real* r = static_cast<const real*>((fi == 0 ? a.halo_src : a.halo_src2)[a.halo_set[bpos]]) + (size_t)hr * REC;
                 const int jn = a.halo_pos[(size_t)bpos * Nfp + i];
                 dp = r[jn] - pm; dnv = -r[Nfp + jn] - nvm;
               } else {

@@ -6,6 +6,7 @@ fetched on the device from the neighbour's trace buffer by `dg_halo_pull` (k_hal
     part = partition_elements(EToV, VX, nparts, weights)         # weighted recursive coordinate bisection
     dd = Decomposition(N, precision, EToV, VX, rho, c, part)     # one DG context per part, halo tables
     dd.bind_torch("cuda:0"); dd.dg_set_source(...); dd.dg_step(n); q = dd.dg_get_fields()
+    dd.rtm_bind(nsteps, xr); data = dd.rtm_forward_shot(nsteps); dd.rtm_backward_shot(nsteps, data); I = dd.rtm_image_read()
 
 The paper partitions with METIS, cell weights 2^(l-1) and keeps the finest cells off the cuts
 (PAPER.md:387); METIS is not in this container: `partition_elements` is a weighted coordinate bisection that takes the same
@@ -130,8 +131,8 @@ class Decomposition:
         EToE, EToF, mapP = g.dg_get_connectivity()
         self.dt = g.dg_get_dt()[0]
         self.level = g.dg_get_levels()
+        self._g = g                                                  # host-only context of the whole mesh (locates receivers)
         self.Np, self.Nfp = g.Np, g.Nfp
-        g.close()
         self.elems = [np.nonzero(self.part == p)[0] for p in range(self.nparts)]
         local = np.full(self.K, -1, dtype=np.int64)
         for e in self.elems:
@@ -250,6 +251,62 @@ class Decomposition:
     def close(self):
         for s in self.sub:
             s.close()
+        self._g.close()
+
+    # ---- RTM on the decomposed mesh: the source and the receiver run share the partition, so the imaging condition needs
+    # no exchange; every sub-domain captures / replays the traces of ITS absorbing faces, records / injects
+    # at ITS receivers and keeps ITS part of the image.  The exchange is the fused one (dg_halo_sources, rtm_halo_sources).
+    def rtm_bind(self, nsteps, xr, device="cuda:0"):
+        """Receivers (global list xr[nr][3]) to the sub-domains that contain them; trace histories for nsteps global steps."""
+        xr = np.asarray(xr, dtype=np.float64).reshape(-1, 3)
+        self._g.dg_set_receivers(xr)
+        self.rcv_sel = [np.nonzero(self.part[self._g.dg_get_receivers()[0]] == p)[0] for p in range(self.nparts)]
+        self.nr = xr.shape[0]
+        for p in self.mine():
+            if self.rcv_sel[p].size:
+                self.sub[p].dg_set_receivers(xr[self.rcv_sel[p]])
+            self.sub[p].bind_history_torch(nsteps, device)
+
+    def _fine_sources(self, m, tr, p):
+        lmin = self.first_level_starting_at(m)
+        return [tr[q][0][lev] if lev >= lmin else tr[q][1] for (q, _, _, _), lev in zip(self.sets[p], self.set_level[p])]
+
+    def rtm_forward_shot(self, nsteps):
+        """Forward phase in lock-step; returns the recorded signals data[nr][nfine + 1] in the order of rtm_bind's list."""
+        total = nsteps * self.nlocal
+        for s in self.sub:
+            s.rtm_forward_part(nsteps, 0, 0)                          # initialise: the trace buffers are the phase's own now
+        data = np.zeros((self.nr, total + 1))
+        for j in range(total):
+            tr = [s.rtm_get_trace_levels(0) for s in self.sub]
+            for p, s in enumerate(self.sub):
+                s.dg_halo_sources(self._fine_sources(j % self.nlocal, tr, p))
+            for p, s in enumerate(self.sub):
+                d = s.rtm_forward_part(nsteps, j, 1)
+                if d is not None:
+                    data[self.rcv_sel[p]] = d
+        return data
+
+    def rtm_backward_shot(self, nsteps, data, updir=(0.0, 0.0, -1.0), imaging=1, first_image_step=0):
+        """Backward phase: both wavefields exchange their halo traces before every fine step, the image stays local."""
+        total = nsteps * self.nlocal
+        for p, s in enumerate(self.sub):
+            s.rtm_backward_part(nsteps, data[self.rcv_sel[p]] if self.rcv_sel[p].size else None, 0, 0, updir, imaging,
+                                first_image_step)
+        for j in range(total):
+            trF = [s.rtm_get_trace_levels(0) for s in self.sub]
+            trR = [s.rtm_get_trace_levels(1) for s in self.sub]
+            for p, s in enumerate(self.sub):
+                s.dg_halo_sources(self._fine_sources(j % self.nlocal, trF, p))
+                s.rtm_halo_sources(self._fine_sources(j % self.nlocal, trR, p))
+            for s in self.sub:
+                s.rtm_backward_part(nsteps, None, j, 1, updir, imaging, first_image_step)
+
+    def rtm_image_read(self):
+        img = np.empty((self.K, self.Np))
+        for p, s in enumerate(self.sub):
+            img[self.elems[p]] = s.rtm_image_read()
+        return img
 
 
 class RankDecomposition(Decomposition):

@@ -219,6 +219,51 @@ def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump,
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("N,precision,nparts,nlevels", [(3, 64, 2, 1), (3, 32, 3, 1), (2, 64, 3, 3), (4, 32, 2, 3), (3, 64, 4, 3)])
+def test_rtm_shot_on_a_decomposed_mesh(N, precision, nparts, nlevels):
+    """Both phases of a shot with the mesh cut into sub-domains: every sub-domain captures and replays the
+    traces of its own absorbing faces, records and injects at its own receivers, keeps its part of the image; the source
+    and - backward - the receiver wavefield exchange halo traces inside the step kernels before every fine step
+    (rtm_forward_part / rtm_backward_part, dg_halo_sources / rtm_halo_sources).  Signals, final state and image equal
+    the single-domain oracle's."""
+    from paper_1506_00907_b200.decomp import Decomposition, partition_elements
+    nsteps = 60 if nlevels == 1 else 32
+    if nlevels == 1:
+        cfg = make_config("cfg4_rtm", hexes=(5, 5, 3), N=N, nsteps=nsteps, n_receivers_side=4)
+    else:
+        cfg = make_config("cfg3_lts", hexes=(5, 5, 6), N=N, nsteps=nsteps)
+        gx = np.linspace(0.4, 2.6, 4)
+        cfg["receivers"] = np.array([[x + 0.013, y + 0.007, 0.06] for x in gx for y in gx])
+        cfg["updir"] = np.array([0.0, 0.0, -1.0])
+    cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
+    o = make_oracle(cfg)
+    lev = np.asarray(o.level)
+    part = partition_elements(cfg["EToV"], cfg["VX"], nparts, 2.0 ** lev)
+    dd = Decomposition(N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part, default_bc=cfg["default_bc"],
+                       nlevels=nlevels, cfl=cfg["cfl"], fused=True)
+    dd.bind_torch("cuda:0")
+    s = cfg["source"]
+    dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+    dd.rtm_bind(nsteps, cfg["receivers"], "cuda:0")
+    assert sum(sel.size > 0 for sel in dd.rcv_sel) >= 2              # the receivers lie in several sub-domains
+    tol = 1e-10 if precision == 64 else 1e-5
+    data_g = dd.rtm_forward_shot(nsteps)
+    data_o, hist, qT = o.rtm_forward(nsteps)
+    assert np.abs(data_o).max() > 0
+    assert rel_l2(data_g, data_o) < tol, rel_l2(data_g, data_o)
+    assert rel_l2(dd.dg_get_fields(), qT) < tol
+    share_q = np.array([np.linalg.norm(qT[part == p]) for p in range(nparts)]) / np.linalg.norm(qT)
+    assert share_q.min() > 1e-3, share_q                              # the wave has crossed every cut
+    dd.rtm_backward_shot(nsteps, data_o, updir=tuple(cfg["updir"]))
+    I_o, FS, FR = o.rtm_backward(nsteps, qT, hist, data_o, updir=cfg["updir"], nglobal_total=nsteps)
+    img = dd.rtm_image_read()
+    share = np.array([np.linalg.norm(I_o[part == p]) for p in range(nparts)]) / np.linalg.norm(I_o)
+    assert np.abs(I_o).max() > 0 and (share > 1e-6).sum() >= 2, share
+    assert rel_l2(img, I_o) < (1e-4 if precision == 32 else 1e-10), rel_l2(img, I_o)
+    dd.close()
+
+
+@pytest.mark.gpu
 def test_halo_and_spill_calls_reject_bad_arguments():
     """Error behaviour stated in include/dgrtm.h: wrong arguments come back as error codes (DGError), nothing aborts."""
     import paper_1506_00907_b200 as pk
