@@ -124,7 +124,7 @@ class Decomposition:
         EToV = np.ascontiguousarray(EToV, dtype=np.int32)
         self.K, self.part = EToV.shape[0], np.asarray(part, dtype=np.int32)
         self.nparts = int(self.part.max()) + 1
-        assert self.nparts <= 9, "a sub-domain has at most 8 halo sets"
+        assert self.nparts <= 33, "a sub-domain has at most 32 halo sets (one per neighbour and level behind the cut)"
         # global connectivity and the global stable step from a host-only context of the whole mesh
         g = DG(N, precision, EToV, VX, face_bc=face_bc, default_bc=default_bc)
         g.dg_set_model(rho, c, self.nlevels, cfl)
