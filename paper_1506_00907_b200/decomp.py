@@ -370,6 +370,70 @@ class RankDecomposition(Decomposition):
     def dg_set_state(self, q, t0=0.0):
         self.sub[self.rank].dg_set_state(q[self.elems[self.rank]], t0)
 
+    # ---- RTM, one process per sub-domain: the fused exchange for both wavefields, a host all-gather per fine step
+    def _field_offsets(self, field):
+        me = self.sub[self.rank]
+        cur, half, _ = me.rtm_get_trace_levels(field)
+        base = me._ws.data_ptr() if field == 0 else me._hist.data_ptr()   # F lives in the workspace, R in the RTM region
+        offs = [None] * self.nparts
+        self.dist.all_gather_object(offs, ([int(c - base) for c in cur], int(half - base)))
+        return offs
+
+    def _peer_sources(self, m, offs, peer):
+        lmin = self.first_level_starting_at(m)
+        return [peer[q].data_ptr() + (offs[q][0][lev] if lev >= lmin else offs[q][1])
+                for (q, _, _, _), lev in zip(self.sets[self.rank], self.set_level[self.rank])]
+
+    def rtm_bind(self, nsteps, xr, device="cuda:0"):
+        from torch.multiprocessing.reductions import reduce_tensor
+        super().rtm_bind(nsteps, xr, device)
+        handles = [None] * self.nparts
+        self.dist.all_gather_object(handles, reduce_tensor(self.sub[self.rank]._hist))
+        self._peer_hist = {}
+        for q, _, _, _ in self.sets[self.rank]:
+            fn, a = handles[q]
+            self._peer_hist[q] = fn(*a)
+        self.dist.barrier()
+
+    def rtm_forward_shot(self, nsteps):
+        import torch
+        me, total = self.sub[self.rank], nsteps * self.nlocal
+        me.rtm_forward_part(nsteps, 0, 0)
+        torch.cuda.synchronize(self._device)
+        mine = None
+        for j in range(total):
+            offs = self._field_offsets(0)               # orders this step after every rank's previous one
+            me.dg_halo_sources(self._peer_sources(j % self.nlocal, offs, self._peer))
+            mine = me.rtm_forward_part(nsteps, j, 1)
+            torch.cuda.synchronize(self._device)
+        parts = [None] * self.nparts
+        self.dist.all_gather_object(parts, mine)
+        data = np.zeros((self.nr, total + 1))
+        for p in range(self.nparts):
+            if parts[p] is not None:
+                data[self.rcv_sel[p]] = parts[p]
+        return data
+
+    def rtm_backward_shot(self, nsteps, data, updir=(0.0, 0.0, -1.0), imaging=1, first_image_step=0):
+        import torch
+        me, total, sel = self.sub[self.rank], nsteps * self.nlocal, self.rcv_sel[self.rank]
+        me.rtm_backward_part(nsteps, data[sel] if sel.size else None, 0, 0, updir, imaging, first_image_step)
+        torch.cuda.synchronize(self._device)
+        for j in range(total):
+            offF, offR = self._field_offsets(0), self._field_offsets(1)
+            me.dg_halo_sources(self._peer_sources(j % self.nlocal, offF, self._peer))
+            me.rtm_halo_sources(self._peer_sources(j % self.nlocal, offR, self._peer_hist))
+            me.rtm_backward_part(nsteps, None, j, 1, updir, imaging, first_image_step)
+            torch.cuda.synchronize(self._device)
+
+    def rtm_image_read(self):
+        parts = [None] * self.nparts
+        self.dist.all_gather_object(parts, self.sub[self.rank].rtm_image_read())
+        img = np.empty((self.K, self.Np))
+        for p in range(self.nparts):
+            img[self.elems[p]] = parts[p]
+        return img
+
     def dg_get_fields(self):
         """Global field on every rank (host all-gather of the sub-domain fields)."""
         mine = self.sub[self.rank].dg_get_fields()

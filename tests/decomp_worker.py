@@ -34,6 +34,40 @@ def run(rank, world, port, N, precision, nsteps, hexes, out_path, workload="cfg2
     dist.destroy_process_group()
 
 
+def run_rtm(rank, world, port, N, precision, nsteps, hexes, out_path, workload):
+    """A whole RTM shot with one process per sub-domain: rank 0 saves the recorded signals, the final state and the image."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    here = os.path.dirname(os.path.abspath(__file__))
+    sys.path.insert(0, os.path.dirname(here))
+    from workloads import make_config
+    from paper_1506_00907_b200.decomp import RankDecomposition, partition_elements
+    cfg = make_config(workload, hexes=hexes, N=N, nsteps=nsteps)
+    cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
+    gx = np.linspace(0.4, 2.6, 4)
+    xr = np.array([[x + 0.013, y + 0.007, 0.06] for x in gx for y in gx])
+    part = partition_elements(cfg["EToV"], cfg["VX"], world)
+    dd = RankDecomposition(dist, N, precision, cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
+                           default_bc=cfg["default_bc"], nlevels=cfg["nlevels"], cfl=cfg["cfl"], fused=True)
+    torch.cuda.set_device(0)
+    dd.bind_torch("cuda:0")
+    s = cfg["source"]
+    dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+    dd.rtm_bind(nsteps, xr, "cuda:0")
+    data = dd.rtm_forward_shot(nsteps)
+    qT = dd.dg_get_fields()
+    dd.rtm_backward_shot(nsteps, data, updir=(0.0, 0.0, -1.0))
+    img = dd.rtm_image_read()
+    if rank == 0:
+        np.savez(out_path, data=data, qT=qT, img=img)
+    dist.barrier()
+    dd.close()
+    dist.destroy_process_group()
+
+
 def check_plan(rank, world, port, N, hexes, out_path):
     """CPU (gloo) check of the one-process-per-sub-domain plan: every rank asks each neighbour - which answers from its OWN
     sub-domain only - for the physical coordinates of the trace-record entries it is going to read, and compares them

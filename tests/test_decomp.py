@@ -324,6 +324,37 @@ def test_one_process_per_sub_domain(N, precision, world, workload, fused, tmp_pa
     assert rel_l2(q, q1) < (1e-13 if precision == 64 else 2e-6), rel_l2(q, q1)
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("N,precision,world,workload", [(3, 64, 2, "cfg2_two_layer"), (2, 64, 3, "cfg3_lts")])
+def test_rtm_shot_one_process_per_sub_domain(N, precision, world, workload, tmp_path):
+    """The whole shot with one process per sub-domain: the step kernels of a rank read both wavefields' halo traces from
+    the CUDA-IPC mappings of its neighbours' workspace (source field) and RTM region (receiver field).  Same signals,
+    final state and image as the single-domain run of the library."""
+    import socket
+    import torch.multiprocessing as mp
+    import decomp_worker
+    nsteps, hexes = (40, (6, 5, 4)) if workload == "cfg2_two_layer" else (24, (5, 5, 6))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "shot.npz")
+    mp.spawn(decomp_worker.run_rtm, args=(world, port, N, precision, nsteps, hexes, out, workload), nprocs=world, join=True)
+    res = np.load(out)
+    cfg = make_config(workload, hexes=hexes, N=N, nsteps=nsteps)
+    cfg["source"] = dict(cfg["source"], f0=60.0, tp=0.01)
+    gx = np.linspace(0.4, 2.6, 4)
+    cfg["receivers"] = np.array([[x + 0.013, y + 0.007, 0.06] for x in gx for y in gx])
+    g = make_gpu(cfg, precision, history_steps=nsteps)
+    data = g.rtm_forward_shot(nsteps)
+    qT = g.rtm_get_fields(0)
+    g.rtm_backward_shot(nsteps, data, updir=(0.0, 0.0, -1.0))
+    img = g.rtm_image_read()
+    g.close()
+    assert np.abs(data).max() > 0 and np.abs(img).max() > 0
+    assert rel_l2(res["data"], data) < 1e-12 and rel_l2(res["qT"], qT) < 1e-12
+    assert rel_l2(res["img"], img) < 1e-11, rel_l2(res["img"], img)
+
+
 @pytest.mark.parametrize("world", [2, 3])
 def test_rank_decomposition_plan_gloo(world, tmp_path):
     """The N > 1 path on the CPU (gloo, world size 2 and 3): every rank's halo requests, answered by the neighbour from its
