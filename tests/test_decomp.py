@@ -296,6 +296,38 @@ def test_halo_and_spill_calls_reject_bad_arguments():
     with pytest.raises(pk.DGError):
         g.dg_set_model_levels(cfg3["rho"], cfg3["c"], 3, 1e-4, np.where(lev == 1, 0, lev))     # neighbours two levels apart
     g.close()
+    # fused exchange and shot phases in parts: one fine step per set of sources, parts in order
+    g = make_gpu(cfg3, 64, history_steps=4)
+    g.dg_halo_sources([])                                            # no halo sets: nothing to name
+    with pytest.raises(pk.DGError) as e:
+        g.dg_step(1)                                                 # 4 fine steps on sources good for one
+    assert e.value.code == pk.DG_ERR_STATE
+    g.dg_step_fine(1)                                                # the failed call did not consume them ... and this one does
+    g.dg_step_fine(3)
+    with pytest.raises(pk.DGError):
+        g.rtm_forward_part(4, 3, 1)                                  # a phase starts at fine step 0
+    g.rtm_forward_part(4, 0, 5)
+    with pytest.raises(pk.DGError):
+        g.rtm_forward_part(4, 4, 1)                                  # parts follow one another
+    with pytest.raises(pk.DGError):
+        g.rtm_backward_part(4, None, 0, 1)                           # no finished forward phase
+    g.rtm_forward_part(4, 5, 11)
+    g.rtm_backward_part(4, None, 0, 0)
+    with pytest.raises(pk.DGError):
+        g.rtm_backward_part(4, None, 2, 1)
+    with pytest.raises(pk.DGError):
+        g.rtm_backward_part(4, None, 0, 17)                          # beyond the phase
+    g.rtm_backward_part(4, None, 0, 16)
+    with pytest.raises(pk.DGError):
+        g.rtm_get_trace_levels(2)
+    g.dg_set_integrator(pk.DG_INTEGRATOR_AB3)
+    g.close()
+    g1 = make_gpu(_cfg(hexes=(3, 3, 2)), 64)
+    g1.dg_set_integrator(pk.DG_INTEGRATOR_LSERK4)
+    with pytest.raises(pk.DGError) as e:
+        g1.dg_halo_sources([])                                       # the fused exchange is in the AB step kernels
+    assert e.value.code == pk.DG_ERR_UNSUPPORTED
+    g1.close()
 
 
 @pytest.mark.gpu
