@@ -331,7 +331,16 @@ class RankDecomposition(Decomposition):
         for q, _, _, _ in self.sets[self.rank]:
             fn, a = handles[q]
             self._peer[q] = fn(*a)                                        # the neighbour's workspace tensor, mapped here
+            self._enable_peer(self._peer[q])
         self.dist.barrier()
+
+    def _enable_peer(self, t):
+        """A mapping that lives on another GPU is read by MY kernels through NVLink: that needs peer access from my device,
+        which torch switches on with the first device-to-device copy between the pair (one GPU in this pool: not exercised)."""
+        import torch
+        mine = torch.device(self._device)
+        if t.device != mine:
+            torch.empty(1, dtype=t.dtype, device=mine).copy_(t.view(-1)[:1])
 
     def _trace_offsets(self):
         """Offsets of every rank's trace buffers (current one per level, half-step one) inside its workspace tensor
@@ -393,6 +402,7 @@ class RankDecomposition(Decomposition):
         for q, _, _, _ in self.sets[self.rank]:
             fn, a = handles[q]
             self._peer_hist[q] = fn(*a)
+            self._enable_peer(self._peer_hist[q])
         self.dist.barrier()
 
     def rtm_forward_shot(self, nsteps):
