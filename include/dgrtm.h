@@ -171,6 +171,10 @@ int dg_set_model_levels(dg_ctx* ctx, const double* rho, const double* c, int nle
 int dg_step_fine(dg_ctx* ctx, int nfine);
 int dg_get_trace_levels(dg_ctx* ctx, void** current /* [nlevels] */, void** half, size_t* nbytes);
 int dg_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device /* [nsets] */);
+/* The three trace buffers of a wavefield (field 0: source / forward, 1: receivers - needs the RTM region): the two that
+ * alternate as a level's current buffer, and the half-step buffer.  Sub-domains that step in lock-step alternate alike, so
+ * a process exchanges these addresses ONCE and derives its neighbour's current buffer from its own (decomp.py). */
+int dg_get_trace_buffers(dg_ctx* ctx, int field, void** buffers /* [3] */, size_t* nbytes);
 
 /* ---- RTM (Fig. 1) ---------------------------------------------------
  * History = boundary traces (p, n.v) of every absorbing boundary face node at every right-hand-side

@@ -63,6 +63,7 @@ SIGNATURES = {
     "dg_step_fine": (_i, [_vp, _i]),
     "dg_get_trace_levels": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_sz)]),
     "dg_halo_sources": (_i, [_vp, _i, C.POINTER(_vp)]),
+    "dg_get_trace_buffers": (_i, [_vp, _i, C.POINTER(_vp), C.POINTER(_sz)]),
     "rtm_set_receiver_capacity": (_i, [_vp, _i64]),
     "rtm_set_spill_packing": (_i, [_vp, _i]),
     "rtm_spill_bytes": (_i, [_vp, _i, C.POINTER(_sz)]),
@@ -268,6 +269,12 @@ class DG:
         cur, half, n = (_vp * 8)(), _vp(), _sz()
         self._ck(_lib.dg_get_trace_levels(self._h, cur, C.byref(half), C.byref(n)))
         return [cur[l] for l in range(L)], half.value, n.value
+
+    def dg_get_trace_buffers(self, field=0):
+        """Device pointers of the two alternating trace buffers and of the half-step buffer of a wavefield."""
+        b, n = (_vp * 3)(), _sz()
+        self._ck(_lib.dg_get_trace_buffers(self._h, int(field), b, C.byref(n)))
+        return [b[0], b[1], b[2]]
 
     def dg_halo_sources(self, src_trace_device):
         """Fused exchange: device pointers of the source buffer of every halo set, for the next (fine) step."""

@@ -458,6 +458,17 @@ int rtm_get_trace_levels(dg_ctx* ctx, int field, void** current, void** half, si
   DG_CATCH(ctx)
 }
 
+int dg_get_trace_buffers(dg_ctx* ctx, int field, void** buffers, size_t* nbytes) {
+  DG_TRY(ctx)
+  if (field == 0) require_bound(ctx); else require_history(ctx);
+  if (field != 0 && field != 1) throw ApiError(DG_ERR_ARG, "field must be 0 (source) or 1 (receivers)");
+  if (!buffers || !nbytes) throw ApiError(DG_ERR_ARG, "buffers / nbytes is NULL");
+  Field& F = field == 0 ? ctx->F : ctx->R;
+  buffers[0] = F.qfb[0]; buffers[1] = F.qfb[1]; buffers[2] = F.qfh;
+  *nbytes = trace_bytes(ctx);
+  DG_CATCH(ctx)
+}
+
 int rtm_halo_sources(dg_ctx* ctx, int nsets, const void* const* src_trace_device) {
   DG_TRY(ctx)
   require_history(ctx);

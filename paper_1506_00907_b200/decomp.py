@@ -332,7 +332,27 @@ class RankDecomposition(Decomposition):
             fn, a = handles[q]
             self._peer[q] = fn(*a)                                        # the neighbour's workspace tensor, mapped here
             self._enable_peer(self._peer[q])
+        self._buf_off = {0: self._gather_buffer_offsets(0, me._ws)}
         self.dist.barrier()
+
+    def _gather_buffer_offsets(self, field, tensor):
+        """Once: every rank's two alternating trace buffers and half-step buffer as offsets inside its shared tensor."""
+        me = self.sub[self.rank]
+        self._my_bufs = getattr(self, "_my_bufs", {})
+        self._my_bufs[field] = me.dg_get_trace_buffers(field)
+        offs = [None] * self.nparts
+        self.dist.all_gather_object(offs, [int(b - tensor.data_ptr()) for b in self._my_bufs[field]])
+        return offs
+
+    def _current_offsets(self, field):
+        """Per rank ([offset of the current buffer of level l], offset of the half-step buffer).  Sub-domains in lock-step
+        alternate their buffers alike: the neighbour's current buffer of a level is the one with MY parity of that level.
+        The barrier orders this fine step after every rank's previous one."""
+        me = self.sub[self.rank]
+        cur = (me.dg_get_trace_levels() if field == 0 else me.rtm_get_trace_levels(field))[0]
+        par = [0 if c == self._my_bufs[field][0] else 1 for c in cur]
+        self.dist.barrier()
+        return [([o[p] for p in par], o[2]) for o in self._buf_off[field]]
 
     def _enable_peer(self, t):
         """A mapping that lives on another GPU is read by MY kernels through NVLink: that needs peer access from my device,
@@ -343,14 +363,7 @@ class RankDecomposition(Decomposition):
             torch.empty(1, dtype=t.dtype, device=mine).copy_(t.view(-1)[:1])
 
     def _trace_offsets(self):
-        """Offsets of every rank's trace buffers (current one per level, half-step one) inside its workspace tensor
-        (a host-side all-gather)."""
-        me = self.sub[self.rank]
-        cur, half, _ = me.dg_get_trace_levels()
-        base = me._ws.data_ptr()
-        offs = [None] * self.nparts
-        self.dist.all_gather_object(offs, ([int(c - base) for c in cur], int(half - base)))
-        return offs
+        return self._current_offsets(0)
 
     def dg_step(self, nsteps):
         import torch
@@ -358,12 +371,12 @@ class RankDecomposition(Decomposition):
         for _ in range(int(nsteps)):
             for m in range(self.nlocal):
                 lmin = self.first_level_starting_at(m)
-                offs = self._trace_offsets()        # also orders this step after every rank's previous step (see below)
+                offs = self._trace_offsets()        # (a barrier: this step comes after every rank's previous one)
                 if self.fused:                      # my step kernel reads the neighbours' buffers; they write the OTHER ones
                     me.dg_halo_sources([self._peer[q].data_ptr() + (offs[q][0][lev] if lev >= lmin else offs[q][1])
                                         for (q, _, _, _), lev in zip(self.sets[self.rank], self.set_level[self.rank])])
                     me.dg_step_fine(1)
-                    torch.cuda.synchronize(self._device)    # my reads and my new traces are complete before the next all-gather
+                    torch.cuda.synchronize(self._device)    # my reads and my new traces are complete before the next barrier
                     continue
                 for i, (q, _, _, _) in enumerate(self.sets[self.rank]):
                     if self.set_mine[self.rank][i] < lmin:
@@ -374,19 +387,14 @@ class RankDecomposition(Decomposition):
                 torch.cuda.synchronize(self._device)    # my fetches have read the neighbours' traces ...
                 self.dist.barrier()                     # ... on every rank, before anybody's step overwrites them
                 me.dg_step_fine(1)
-                torch.cuda.synchronize(self._device)    # my new traces are complete before the next all-gather returns
+                torch.cuda.synchronize(self._device)    # my new traces are complete before the next barrier returns
 
     def dg_set_state(self, q, t0=0.0):
         self.sub[self.rank].dg_set_state(q[self.elems[self.rank]], t0)
 
-    # ---- RTM, one process per sub-domain: the fused exchange for both wavefields, a host all-gather per fine step
+    # ---- RTM, one process per sub-domain: the fused exchange for both wavefields, a host barrier per fine step
     def _field_offsets(self, field):
-        me = self.sub[self.rank]
-        cur, half, _ = me.rtm_get_trace_levels(field)
-        base = me._ws.data_ptr() if field == 0 else me._hist.data_ptr()   # F lives in the workspace, R in the RTM region
-        offs = [None] * self.nparts
-        self.dist.all_gather_object(offs, ([int(c - base) for c in cur], int(half - base)))
-        return offs
+        return self._current_offsets(field)
 
     def _peer_sources(self, m, offs, peer):
         lmin = self.first_level_starting_at(m)
@@ -403,6 +411,7 @@ class RankDecomposition(Decomposition):
             fn, a = handles[q]
             self._peer_hist[q] = fn(*a)
             self._enable_peer(self._peer_hist[q])
+        self._buf_off[1] = self._gather_buffer_offsets(1, self.sub[self.rank]._hist)
         self.dist.barrier()
 
     def rtm_forward_shot(self, nsteps):
