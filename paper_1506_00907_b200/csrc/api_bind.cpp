@@ -204,7 +204,8 @@ int dg_bind_workspace(dg_ctx* ctx, void* dptr, size_t n, void* cuda_stream) {
   {
     const size_t nbf = ctx->mesh.bnd_k.size();
     ctx->h_hrec.assign(nbf, -1); ctx->h_hset.assign(nbf, 0); ctx->h_hpos.assign(nbf * ctx->Nfp, 0);
-    ctx->halo_src_valid = false;
+    if (nbf) upload_raw(ctx, ctx->d_halo_face, ctx->h_hrec.data(), nbf * 8);   // -1: no face is a halo face yet
+    ctx->halo_src_valid = false; ctx->halo_src2_valid = false;
   }
   ctx->have_final = false; ctx->have_backward = false;
   sync_stream(ctx);
