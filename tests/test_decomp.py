@@ -219,7 +219,8 @@ def test_decomposed_multirate_run_matches_the_oracle(N, precision, nparts, lump,
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N,precision,nparts,nlevels", [(3, 64, 2, 1), (3, 32, 3, 1), (2, 64, 3, 3), (4, 32, 2, 3), (3, 64, 4, 3)])
+@pytest.mark.parametrize("N,precision,nparts,nlevels", [(3, 64, 2, 1), (3, 32, 3, 1), (2, 64, 3, 3), (4, 32, 2, 3), (3, 64, 4, 3),
+                                                        (1, 64, 3, 3), (5, 64, 2, 1)])      # the last two: k_step, two fields
 def test_rtm_shot_on_a_decomposed_mesh(N, precision, nparts, nlevels):
     """Both phases of a shot with the mesh cut into sub-domains: every sub-domain captures and replays the
     traces of its own absorbing faces, records and injects at its own receivers, keeps its part of the image; the source
