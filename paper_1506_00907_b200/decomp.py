@@ -199,14 +199,10 @@ class Decomposition:
         self._bound = True
 
     def dg_set_source(self, x0, f0, tp, amp=1.0):
-        """The point source goes to the sub-domain that contains it (lowest part id on a tie)."""
-        for s in self.sub:
-            try:
-                s.dg_set_source(x0, f0, tp, amp)
-                return
-            except Exception:
-                continue
-        raise ValueError("source outside the mesh")
+        """The point source goes to the sub-domain that holds the element the whole mesh locates it in (reading Q11:
+        lowest element id that contains the point); DGError if it lies outside the mesh."""
+        self._g.dg_set_source(x0, f0, tp, amp)
+        self.sub[int(self.part[self._g.dg_get_source()[0]])].dg_set_source(x0, f0, tp, amp)
 
     def dg_set_state(self, q, t0=0.0):
         for p, s in enumerate(self.sub):
