@@ -252,8 +252,9 @@ class Decomposition:
     # ---- RTM on the decomposed mesh: the source and the receiver run share the partition, so the imaging condition needs
     # no exchange; every sub-domain captures / replays the traces of ITS absorbing faces, records / injects
     # at ITS receivers and keeps ITS part of the image.  The exchange is the fused one (dg_halo_sources, rtm_halo_sources).
-    def rtm_bind(self, nsteps, xr, device="cuda:0"):
-        """Receivers (global list xr[nr][3]) to the sub-domains that contain them; trace histories for nsteps global steps."""
+    def rtm_bind(self, nsteps, xr, device="cuda:0", spill_window=0):
+        """Receivers (global list xr[nr][3]) to the sub-domains that contain them; trace histories for nsteps global steps
+        (spill_window > 0: in pinned host memory behind a device ring of that many records, rtm_set_trace_spill)."""
         xr = np.asarray(xr, dtype=np.float64).reshape(-1, 3)
         self._g.dg_set_receivers(xr)
         self.rcv_sel = [np.nonzero(self.part[self._g.dg_get_receivers()[0]] == p)[0] for p in range(self.nparts)]
@@ -261,6 +262,8 @@ class Decomposition:
         for p in self.mine():
             if self.rcv_sel[p].size:
                 self.sub[p].dg_set_receivers(xr[self.rcv_sel[p]])
+            if spill_window:
+                self.sub[p].spill_traces_torch(nsteps, spill_window)
             self.sub[p].bind_history_torch(nsteps, device)
 
     def _fine_sources(self, m, tr, p):
@@ -397,9 +400,9 @@ class RankDecomposition(Decomposition):
         return [peer[q].data_ptr() + (offs[q][0][lev] if lev >= lmin else offs[q][1])
                 for (q, _, _, _), lev in zip(self.sets[self.rank], self.set_level[self.rank])]
 
-    def rtm_bind(self, nsteps, xr, device="cuda:0"):
+    def rtm_bind(self, nsteps, xr, device="cuda:0", spill_window=0):
         from torch.multiprocessing.reductions import reduce_tensor
-        super().rtm_bind(nsteps, xr, device)
+        super().rtm_bind(nsteps, xr, device, spill_window)
         handles = [None] * self.nparts
         self.dist.all_gather_object(handles, reduce_tensor(self.sub[self.rank]._hist))
         self._peer_hist = {}
