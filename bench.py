@@ -595,6 +595,38 @@ def extra_decomposition(torch, device, hexes, T=200):
     return out
 
 
+def extra_decomposed_shot(torch, device, hexes, nsteps):
+    """One RTM shot of config 4 with the mesh cut into 1, 2 and 4 sub-domains that share this GPU (decomp.py: the phases in
+    parts, both wavefields' halo traces read inside the step kernels).  What the cuts cost before any NVLink
+    is involved, and that the image does not depend on them."""
+    from workloads import make_config
+    from paper_1506_00907_b200.decomp import Decomposition, partition_elements
+    cfg = make_config("cfg4_rtm", hexes=hexes, nsteps=nsteps)
+    out = []
+    for nparts in (1, 2, 4):
+        part = partition_elements(cfg["EToV"], cfg["VX"], nparts)
+        dd = Decomposition(cfg["N"], cfg["precision"], cfg["EToV"], cfg["VX"], cfg["rho"], cfg["c"], part,
+                           default_bc=cfg["default_bc"], cfl=cfg["cfl"], fused=True)
+        dd.bind_torch(device)
+        s = cfg["source"]
+        dd.dg_set_source(s["x0"], s["f0"], s["tp"], s["amp"])
+        dd.rtm_bind(nsteps, cfg["receivers"], device)
+        torch.cuda.synchronize(device)
+        t0 = time.perf_counter()
+        data = dd.rtm_forward_shot(nsteps)
+        torch.cuda.synchronize(device)
+        t1 = time.perf_counter()
+        dd.rtm_backward_shot(nsteps, data, updir=tuple(cfg["updir"]))
+        torch.cuda.synchronize(device)
+        t2 = time.perf_counter()
+        img = dd.rtm_image_read()
+        out.append({"workload": "cfg4_rtm", "K": int(dd.K), "nsteps": nsteps, "sub_domains": nparts,
+                    "forward_us_per_step": round((t1 - t0) / nsteps * 1e6, 1),
+                    "backward_us_per_step": round((t2 - t1) / nsteps * 1e6, 1), "image_l2": float(np.linalg.norm(img))})
+        dd.close()
+    return out
+
+
 def survey_shots(nshots, lengths, hexes, receivers):
     """Seeded shot list of a survey over one mesh ("29 gathers"): sources along a line at the top, each
     with its own receiver set (a shifted sub-grid, so the counts differ between gathers)."""
@@ -771,6 +803,7 @@ def run_ours(args):
         line["unfused_kernels"] = extra_unfused_kernels(torch, device, peak, None if big else (8, 8, 4), traffic_table)
         line["cfg5_sweep"] = extra_cfg5_sweep(torch, device, peak, None if big else (8, 8, 8), alu=line["peaks"])
         line["decomposition_one_gpu"] = extra_decomposition(torch, device, None if big else (8, 8, 4), 200 if big else 10)
+        line["decomposed_rtm_shot_one_gpu"] = extra_decomposed_shot(torch, device, None if big else (8, 8, 4), 200 if big else 10)
         line["rtm_shot"] = extra_rtm_shot(torch, device, peak, peak_src, None if big else (8, 8, 4),
                                           None if big else 20, traffic_table)
     if rank == 0:
