@@ -221,7 +221,8 @@ int rtm_backward_shot(dg_ctx* ctx, int nsteps, const double* data, const double 
  * steps.  The part with fine0 = 0 initialises the phase exactly as the _shot call does (data / updir / imaging are read
  * then and on every part; data may be NULL after the first), the part that reaches nsteps * 2^(L-1) finishes it (final
  * capture and sample, data_out; earlier parts ignore data_out and do not synchronise).  An empty part at 0 (nfine = 0)
- * initialises alone - the trace buffers can then be asked for before the first step.  The parts follow one another
+ * initialises alone - the trace buffers can then be asked for before the first step (a backward part at 0 that carries
+ * signals always starts the phase anew).  The parts follow one another
  * (DG_ERR_STATE otherwise).  rtm_forward_shot(n, d) = rtm_forward_part(n, 0, n * 2^(L-1), d), likewise backward.
  * rtm_get_trace_levels: dg_get_trace_levels for field 0 (source wavefield) or 1 (receiver wavefield).
  * rtm_halo_sources: dg_halo_sources for the receiver wavefield; a two-field step needs both, each for ONE fine step. */

@@ -387,7 +387,7 @@ static void backward_part(dg_ctx* ctx, int nsteps, const double* data, const dou
   if (imaging < 0 || imaging > 3) throw ApiError(DG_ERR_ARG, "unknown imaging condition");
   const int64_t ntot = ctx->final_nsteps, total = (int64_t)nsteps * ctx->nlocal;
   if (fine0 < 0 || nfine < 0 || fine0 + nfine > total) throw ApiError(DG_ERR_ARG, "fine steps outside the backward phase");
-  if (fine0 == 0 && !(ctx->part_phase == 2 && ctx->part_nsteps == nsteps && ctx->part_fresh)) {
+  if (fine0 == 0 && (data || !(ctx->part_phase == 2 && ctx->part_nsteps == nsteps && ctx->part_fresh))) {   // (signals given: a new start)
     if (!data && ctx->nr > 0 && !ctx->data_valid)
       throw ApiError(DG_ERR_STATE, "the signals on the device belong to another receiver set: pass data");
     if (data) ctx->data_valid = true;
